@@ -1,0 +1,229 @@
+"""Pins for the brute-force oracle (oracle/): it is checked against what the paper and the
+mathematics fix, not against itself.
+
+Eq. 1 + Gaussian kernel truncated at sphere_radius.
+Each test names the mistake it is meant to catch.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+from hypothesis import given, settings, strategies as st
+
+from paper_2012_13173_b200 import workloads
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+AM = 1.0 / 60.0
+
+
+def vec_dist(lon1, lat1, lon2, lat2):
+    """Independent great-circle formula: atan2(|a x b|, a . b) on fp64 unit vectors
+    (textbook; shares nothing with the oracle's haversine)."""
+    l1, b1, l2, b2 = map(np.deg2rad, (lon1, lat1, lon2, lat2))
+    a = np.stack([np.cos(b1) * np.cos(l1), np.cos(b1) * np.sin(l1), np.sin(b1)], -1)
+    b = np.stack([np.cos(b2) * np.cos(l2), np.cos(b2) * np.sin(l2), np.sin(b2)], -1)
+    a, b = np.broadcast_arrays(a, b)
+    return np.arctan2(np.linalg.norm(np.cross(a, b), axis=-1), (a * b).sum(-1))
+
+
+# ---------------------------------------------------------------- distance (reading c3)
+def test_distance_closed_forms(oracle):
+    # same meridian: d = |dlat|   (catches a missing 1/2 in the haversine, deg/rad slips)
+    assert oracle.distance(10.0, -20.0, 10.0, 35.0) == pytest.approx(math.radians(55.0), abs=1e-15)
+    # both on the equator: d = |dlon|, including across the 0/360 seam
+    assert oracle.distance(3.0, 0.0, 47.0, 0.0) == pytest.approx(math.radians(44.0), abs=1e-15)
+    assert oracle.distance(359.5, 0.0, 0.25, 0.0) == pytest.approx(math.radians(0.75), abs=1e-15)
+    # across the pole: (l, 89.9) to (l+180, 89.9) is 0.2 deg  (catches a dropped cos factor)
+    assert oracle.distance(12.0, 89.9, 192.0, 89.9) == pytest.approx(math.radians(0.2), abs=1e-13)
+    # 1 deg of longitude at lat 60 is NOT 0.5 deg exactly: spherical law of cosines value
+    d = math.acos(math.sin(math.radians(60)) ** 2 + math.cos(math.radians(60)) ** 2 * math.cos(math.radians(1)))
+    assert oracle.distance(0.0, 60.0, 1.0, 60.0) == pytest.approx(d, rel=1e-9)
+    # symmetric, zero on the diagonal, antipode = pi
+    assert oracle.distance(5, 6, 7, 8) == oracle.distance(7, 8, 5, 6)
+    assert oracle.distance(123.4, -56.7, 123.4, -56.7) == 0.0
+    assert oracle.distance(0.0, 0.0, 180.0, 0.0) == pytest.approx(math.pi, abs=1e-12)
+
+
+def test_distance_vs_vector_formula_near_pairs(oracle):
+    rng = np.random.default_rng(7)
+    lon1 = rng.uniform(0, 360, 20000)
+    lat1 = np.degrees(np.arcsin(rng.uniform(-1, 1, 20000)))
+    lon2 = lon1 + rng.uniform(-0.2, 0.2, 20000) / np.maximum(np.cos(np.deg2rad(lat1)), 0.05)
+    lat2 = np.clip(lat1 + rng.uniform(-0.2, 0.2, 20000), -90, 90)
+    ref = vec_dist(lon1, lat1, lon2, lat2)
+    got = np.array([oracle.distance(a, b, c, d) for a, b, c, d in zip(lon1, lat1, lon2, lat2)])
+    # both formulas are conditioned to ~1e-16 absolute on unit vectors at these separations
+    assert np.max(np.abs(got - ref)) < 2e-15 + 1e-12 * np.max(ref)
+
+
+# ---------------------------------------------------------------- hand case (golden)
+def test_hand_3x3_golden(oracle):
+    rows = np.loadtxt(os.path.join(GOLDEN, "hand_3x3.txt"))
+    clon, clat = rows[:, 0] * AM, rows[:, 1] * AM
+    slon = np.array([0, 1, 0, -1, 10]) * AM
+    slat = np.array([0, 0, -1, 1, 10]) * AM
+    val = np.array([1, 2, 4, 8, 100], dtype=np.float32)
+    r = oracle.grid(1.0 * AM, 1.2 * AM, clon, clat, slon, slat, val)
+    assert np.array_equal(r.counts, rows[:, 2].astype(np.int64))
+    np.testing.assert_allclose(r.weightmap, rows[:, 3], rtol=1e-6)
+    np.testing.assert_allclose(r.datacube[:, 0], rows[:, 4], rtol=1e-6)
+    assert np.all(r.near_boundary == 0)
+
+
+# ---------------------------------------------------------------- kernel + normalisation (c1, c5)
+def test_single_sample_reproduces_gaussian_weight_map(oracle):
+    sig, R = 2.0 * AM, 7.2 * AM   # no cell sits exactly on the boundary
+    # cells on the sample's meridian: d = |dlat| in closed form (no distance code involved)
+    off = np.linspace(-9, 9, 37) * AM
+    clat = 40.0 + off
+    clon = np.full_like(clat, 77.0)
+    r = oracle.grid(sig, R, clon, clat, [77.0], [40.0], np.array([3.25], np.float32))
+    d = np.abs(off)
+    inside = d <= R
+    expect = np.where(inside, np.exp(-np.deg2rad(d) ** 2 / (2 * np.deg2rad(sig) ** 2)), 0.0)
+    np.testing.assert_allclose(r.weightmap, expect, rtol=1e-12, atol=0)
+    assert np.array_equal(r.counts, inside.astype(np.int64))
+    np.testing.assert_allclose(r.datacube[inside, 0], 3.25, rtol=4e-16)   # V = v wherever W > 0
+    assert np.all(np.isnan(r.datacube[~inside, 0]))       # c5: empty cell -> NaN
+    assert np.all(r.weightmap[~inside] == 0.0)
+    # peak is 1 (no 1/(2 pi sigma^2) factor, reading c1)
+    assert r.weightmap[off == 0][0] == 1.0
+    # cells on the equator: d = |dlon| in closed form
+    clon2 = 200.0 + off
+    r2 = oracle.grid(sig, R, clon2, np.zeros_like(clon2), [200.0], [0.0], np.array([1.0], np.float32))
+    d2 = np.abs(clon2 - 200.0)          # the representable offsets (200 + off rounds at 3e-14 deg)
+    expect2 = np.where(d2 <= R, np.exp(-np.deg2rad(d2) ** 2 / (2 * np.deg2rad(sig) ** 2)), 0.0)
+    np.testing.assert_allclose(r2.weightmap, expect2, rtol=1e-12)
+
+
+def test_constant_field_grids_to_constant(oracle):
+    w = workloads.make(1, scale=0.05)
+    clon, clat = w.target.cell_centers()
+    const = np.full((w.n, 1), 2.718281828, dtype=np.float32)
+    r = oracle.grid(w.sigma_deg, w.radius_deg, clon, clat, w.lon, w.lat, const)
+    ok = r.weightmap > 0
+    assert ok.sum() > 0.9 * ok.size
+    np.testing.assert_allclose(r.datacube[ok, 0], float(const[0, 0]), rtol=1e-15)
+    np.testing.assert_allclose(r.absmap[ok, 0], float(const[0, 0]), rtol=1e-15)
+
+
+def test_permutation_invariance(oracle):
+    w = workloads.make(1, scale=0.05)
+    clon, clat = w.target.cell_centers()
+    r0 = oracle.grid(w.sigma_deg, w.radius_deg, clon, clat, w.lon, w.lat, w.values)
+    p = np.random.default_rng(3).permutation(w.n)
+    r1 = oracle.grid(w.sigma_deg, w.radius_deg, clon, clat, w.lon[p], w.lat[p], w.values[p])
+    assert np.array_equal(r0.counts, r1.counts)
+    np.testing.assert_allclose(r1.weightmap, r0.weightmap, rtol=1e-15)
+    np.testing.assert_allclose(r1.datacube, r0.datacube, rtol=0, atol=1e-14 * np.nanmax(r0.absmap))
+
+
+def test_rotation_about_pole_axis_and_seam(oracle):
+    """Adding a constant to every longitude leaves the result unchanged; moving the patch
+    onto the 0/360 seam exercises the wrap (catches a missing remainder / wrong sign)."""
+    lon, lat, val, wts, clon, clat = workloads.random_case(1, 400, 60, 100.0, 55.0, 0.3)
+    sig, R = 3 * AM, 9 * AM
+    r0 = oracle.grid(sig, R, clon, clat, lon, lat, val)
+    shift = 260.0 - 0.1     # patch now straddles lon = 0
+    r1 = oracle.grid(sig, R, np.mod(clon + shift, 360), clat, np.mod(lon + shift, 360), lat, val)
+    assert r0.counts.sum() > 0
+    # the shift is not exact in fp64 (1 ulp of 360 = 6e-14 deg ~ 1e-15 rad): tolerance 1e-9 rel
+    ok = r0.near_boundary == 0
+    assert np.array_equal(r0.counts[ok], r1.counts[ok])
+    np.testing.assert_allclose(r1.weightmap[ok], r0.weightmap[ok], rtol=1e-9)
+
+
+# ---------------------------------------------------------------- brute force by another route
+@settings(max_examples=25, deadline=None)
+@given(seed=st.integers(0, 10_000), lat_c=st.sampled_from([0.0, 33.0, -61.0, 84.0, 89.7, -89.9]),
+       lon_c=st.sampled_from([0.05, 180.0, 359.97]), nchan=st.sampled_from([1, 3]),
+       use_w=st.booleans())
+def test_brute_force_numpy_vector_formula(oracle, seed, lat_c, lon_c, nchan, use_w):
+    """Eq. 1 re-evaluated with numpy broadcasting and the VECTOR distance formula
+    (a different route to d), math.fsum-free plain float64 sums: counts equal away from
+    the boundary, W and V to 1e-11."""
+    lon, lat, val, wts, clon, clat = workloads.random_case(seed, 300, 25, lon_c, lat_c, 0.25,
+                                                           nchan=nchan, with_weights=use_w)
+    sig, R = 4 * AM, 10 * AM
+    r = oracle.grid(sig, R, clon, clat, lon, lat, val, wts)
+    d = vec_dist(clon[:, None], clat[:, None], lon[None, :], lat[None, :])
+    Rr, sr = np.deg2rad(R), np.deg2rad(sig)
+    inside = d <= Rr
+    q = np.ones(lon.size) if wts is None else wts.astype(np.float64)
+    w = np.where(inside, np.exp(-d * d / (2 * sr * sr)), 0.0) * q[None, :]
+    W = w.sum(1)
+    S = w @ val.astype(np.float64)
+    band = (np.abs(d - Rr) < 1e-9).sum(1)
+    assert np.all(np.abs(inside.sum(1) - r.counts) <= band)
+    np.testing.assert_allclose(r.weightmap, W, rtol=1e-11, atol=1e-300)
+    ok = W > 0
+    np.testing.assert_allclose(r.datacube[ok], S[ok] / W[ok, None], rtol=0,
+                               atol=1e-11 * max(1.0, float(np.nanmax(r.absmap[ok]))))
+    assert np.all(np.isnan(r.datacube[~ok]))
+
+
+# ---------------------------------------------------------------- weights (c6) and channels (c7)
+def test_weight_semantics(oracle):
+    lon, lat, val, wts, clon, clat = workloads.random_case(5, 500, 40, 10.0, -30.0, 0.3,
+                                                           with_weights=True)
+    sig, R = 3 * AM, 9 * AM
+    base = oracle.grid(sig, R, clon, clat, lon, lat, val)
+    k = oracle.grid(sig, R, clon, clat, lon, lat, val, np.full(lon.size, 2.5, np.float32))
+    np.testing.assert_allclose(k.weightmap, 2.5 * base.weightmap, rtol=1e-14)
+    ok = base.weightmap > 0
+    np.testing.assert_allclose(k.datacube[ok], base.datacube[ok], rtol=0, atol=1e-13)
+    assert np.array_equal(k.counts, base.counts)
+    # q in {0,1}: same W, V as dropping the zero-weight samples; count stays geometric
+    m = np.random.default_rng(1).random(lon.size) < 0.6
+    z = oracle.grid(sig, R, clon, clat, lon, lat, val, m.astype(np.float32))
+    dpd = oracle.grid(sig, R, clon, clat, lon[m], lat[m], val[m])
+    np.testing.assert_allclose(z.weightmap, dpd.weightmap, rtol=1e-14)
+    ok2 = dpd.weightmap > 0
+    np.testing.assert_allclose(z.datacube[ok2], dpd.datacube[ok2], rtol=0, atol=1e-13)
+    assert np.array_equal(z.counts, base.counts)
+    # general weights: W is linear in q
+    a = oracle.grid(sig, R, clon, clat, lon, lat, val, wts)
+    b = oracle.grid(sig, R, clon, clat, lon, lat, val, (2 * wts).astype(np.float32))
+    np.testing.assert_allclose(b.weightmap, 2 * a.weightmap, rtol=1e-14)
+
+
+def test_multichannel_is_per_channel(oracle):
+    lon, lat, val, wts, clon, clat = workloads.random_case(9, 300, 30, 250.0, 12.0, 0.2, nchan=5)
+    sig, R = 3 * AM, 9 * AM
+    full = oracle.grid(sig, R, clon, clat, lon, lat, val)
+    for k in range(5):
+        one = oracle.grid(sig, R, clon, clat, lon, lat, val[:, k].copy())
+        assert np.array_equal(np.isnan(one.datacube[:, 0]), np.isnan(full.datacube[:, k]))
+        ok = one.weightmap > 0
+        assert np.array_equal(one.datacube[ok, 0], full.datacube[ok, k])
+        assert np.array_equal(one.weightmap, full.weightmap)
+
+
+# ---------------------------------------------------------------- boundary, empties, errors (c4)
+def test_support_boundary_and_band(oracle):
+    sig, R = 1.0, 3.0      # degrees; meridian pairs so d = |dlat| in closed form
+    eps_deg = math.degrees(5e-10)
+    clat = np.array([0.0, 0.0, 0.0, 0.0])
+    slat = np.array([R - 10 * eps_deg, R - eps_deg, R + eps_deg, R + 10 * eps_deg])
+    for i, (inside, band) in enumerate([(1, 0), (1, 1), (0, 1), (0, 0)]):
+        r = oracle.grid(sig, R, [5.0], [0.0], [5.0], [slat[i]], np.array([1.0], np.float32))
+        assert r.counts[0] == inside and r.near_boundary[0] == band
+
+
+def test_empty_inputs_and_errors(oracle):
+    r = oracle.grid(1 * AM, 3 * AM, [1.0, 2.0], [3.0, 4.0], [], [], np.zeros((0, 1), np.float32))
+    assert np.all(r.weightmap == 0) and np.all(r.counts == 0) and np.all(np.isnan(r.datacube))
+    r = oracle.grid(1 * AM, 3 * AM, [], [], [1.0], [1.0], np.ones((1, 1), np.float32))
+    assert r.weightmap.size == 0
+    with pytest.raises(ValueError):
+        oracle.grid(0.0, 1.0, [0.0], [0.0], [0.0], [0.0], np.ones(1, np.float32))
+    with pytest.raises(ValueError):
+        oracle.grid(1.0, -1.0, [0.0], [0.0], [0.0], [0.0], np.ones(1, np.float32))
+
+
+def test_duplicates_all_count(oracle):
+    r = oracle.grid(1.0, 3.0, [0.0], [0.0], [0.5] * 4, [0.0] * 4, np.array([1, 2, 3, 6], np.float32))
+    assert r.counts[0] == 4
+    assert r.datacube[0, 0] == pytest.approx(3.0, rel=1e-15)
+    assert r.weightmap[0] == pytest.approx(4 * math.exp(-0.5 * 0.25), rel=1e-14)
