@@ -1,0 +1,156 @@
+/* hcgrid.h -- C-ABI of the B200-native HCGrid hot path (arXiv 2012.13173).
+ *
+ * What the library computes (Sect. 2.1, Eq. 1): for every target
+ * cell g_ij with centre (alpha_ij, delta_ij)
+ *
+ *     V[g_ij] = (1 / W_ij) * sum_n V[s_n] * w(alpha_ij, delta_ij; alpha_n, delta_n)
+ *     W_ij    = sum_n w(alpha_ij, delta_ij; alpha_n, delta_n)
+ *
+ * with the kernel of PAPER.md:186 (Sect. 3.6 iii): a radially symmetric Gaussian of
+ * standard deviation sigma_kernel, w(d) = exp(-d^2 / (2 sigma^2)) of the great-circle
+ * distance d, truncated at "sphere_radius" (d <= R contributes).  Contributing samples
+ * are found through the pre-ordering of PAPER.md:108-124 (Sect. 3.3: HEALPix RING pixel
+ * index per sample, key-value sort, ring table R_start and per-pixel table
+ * P_i -> S_start) and the search of PAPER.md:134-140 (Sect. 3.4 i-v).  Every step runs on
+ * the device; there is no CPU search stage and no CPU fallback.
+ *
+ * Conventions
+ *   - Angles at the boundary are DEGREES (the paper speaks degrees/arcmin/arcsec,
+ *     PAPER.md:24, 218); lon is any real (reduced mod 360), lat in [-90, 90].
+ *   - Unless a function says "HOST", every array pointer is a DEVICE pointer on the
+ *     context's device, owned by the caller, not modified unless it is an output.
+ *   - Flat cell index of a plate-carree target is iy*nx + ix; datacube is
+ *     [ncell][nchan] with the channel fastest (values is [n][nchan] likewise).
+ *   - Empty cell (W == 0): V = NaN, W = 0, count = 0.
+ *   - Per-sample weights q_s multiply the kernel (W = sum q w, V = sum q w v / W);
+ *     counts are geometric (number of samples with d <= R, whatever q).
+ *   - All calls return an hcgrid_status (0 = OK, negative = error); nothing aborts or
+ *     throws.  hcgrid_last_error() gives the message of the last failing call.
+ *   - A context is not re-entrant: one host thread at a time per context.
+ *   - hcgrid_grid() is asynchronous on `stream`; outputs are valid once the stream is
+ *     synchronised.  The context owns all scratch (grow-only, reused across calls).
+ */
+#ifndef HCGRID_H
+#define HCGRID_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hcgrid_ctx hcgrid_ctx;
+
+typedef enum {
+    HCGRID_OK = 0,
+    HCGRID_ERR_INVALID_ARG = -1,
+    HCGRID_ERR_NO_TARGET = -2,
+    HCGRID_ERR_ALLOC = -3,
+    HCGRID_ERR_CUDA = -4,
+    HCGRID_ERR_UNSUPPORTED = -5
+} hcgrid_status;
+
+/* precision mode: pair arithmetic + accumulation + output dtype */
+enum { HCGRID_F32 = 0, HCGRID_F64 = 1 };
+
+/* tuning / debug options for hcgrid_set_option (all have measured defaults) */
+enum {
+    HCGRID_OPT_PROFILE = 1,      /* 1: time every stage with CUDA events (hcgrid_get_stats) */
+    HCGRID_OPT_SUBPIX_BITS = 2,  /* log2 of lookup bins per HEALPix pixel along the ring; -1 = auto.
+                                    Takes effect at the next hcgrid_set_target_*. */
+    HCGRID_OPT_COARSEN = 3,      /* cells per warp task (thread coarsening); 0 = auto */
+    HCGRID_OPT_KERNEL = 4,       /* 0 = auto; 1 = force the simple (non-staged) single-channel kernel;
+                                    2 = force the fp64 pair arithmetic with the F32 output type;
+                                    3 = force the general (any nchan) kernel with fp32 pair arithmetic */
+    HCGRID_OPT_WARPS_PER_SM = 5  /* resident convolution warps per SM; 0 = auto */
+};
+
+typedef struct {
+    int64_t n_samples;        /* samples passed to the last hcgrid_grid                      */
+    int64_t n_kept;           /* samples inside the target's reach (sorted, packed)          */
+    int64_t n_bins;           /* entries of the per-pixel offset table                        */
+    int32_t n_rings;          /* rings of the ring table                                      */
+    int32_t subpix_bits;      /* lookup bins per HEALPix pixel = 2^subpix_bits (may be < 0)   */
+    int32_t coarsen;          /* cells per warp task used                                     */
+    int32_t kernel;           /* convolution kernel variant that ran          */
+    int32_t gpu_launches;     /* kernels launched by the last hcgrid_grid                     */
+    int32_t reserved;
+    float us_pixelise, us_sort, us_tables, us_pack, us_convolve, us_total; /* PROFILE only   */
+} hcgrid_stats;
+
+/* Create a context.  sigma_deg = kernel standard deviation, support_radius_deg =
+ * "sphere_radius", nside = HEALPix partition level N_side,
+ * a power of two in [1, 8192].  precision = HCGRID_F32 or HCGRID_F64.  device = CUDA
+ * ordinal.  On failure *out is NULL and the message is available through
+ * hcgrid_last_error(NULL). */
+int hcgrid_create(hcgrid_ctx** out, double sigma_deg, double support_radius_deg,
+                  int64_t nside, int precision, int device);
+int hcgrid_destroy(hcgrid_ctx* ctx);
+
+int hcgrid_set_option(hcgrid_ctx* ctx, int option, int64_t value);
+
+/* Target = plate-carree grid: cell (ix, iy) centre = (lon0 + ix*dlon, lat0 + iy*dlat),
+ * each evaluated with one rounding per operation (no FMA); dlon, dlat may be negative,
+ * not zero.  Builds the per-row search tables on the device (synchronises the device). */
+int hcgrid_set_target_car(hcgrid_ctx* ctx, int32_t nx, int32_t ny, double lon0_deg,
+                          double lat0_deg, double dlon_deg, double dlat_deg);
+/* Target = arbitrary cells; lon_deg/lat_deg are DEVICE arrays [ncell] (copied). */
+int hcgrid_set_target_cells(hcgrid_ctx* ctx, int64_t ncell, const double* lon_deg,
+                            const double* lat_deg, void* stream);
+
+/* Grid n samples onto the target.
+ *   lon_deg, lat_deg [n] double; values [n][nchan] float; weights [n] float or NULL.
+ *   datacube [ncell][nchan], weightmap [ncell]: float (F32) or double (F64).
+ *   counts [ncell] int32 or NULL.  stream: cudaStream_t (NULL = default stream).
+ * n = 0 is legal (every cell empty). */
+int hcgrid_grid(hcgrid_ctx* ctx, int64_t n, const double* lon_deg, const double* lat_deg,
+                const float* values, int32_t nchan, const float* weights,
+                void* datacube, void* weightmap, int32_t* counts, void* stream);
+
+/* Same call with HOST buffers (pinned or pageable): copies the inputs to context-owned
+ * device buffers, grids, copies the outputs back and synchronises before returning. */
+int hcgrid_grid_host(hcgrid_ctx* ctx, int64_t n, const double* lon_deg, const double* lat_deg,
+                     const float* values, int32_t nchan, const float* weights,
+                     void* datacube, void* weightmap, int32_t* counts);
+
+int64_t hcgrid_ncell(const hcgrid_ctx* ctx);      /* cells of the current target, 0 if none */
+int hcgrid_get_stats(const hcgrid_ctx* ctx, hcgrid_stats* out);
+const char* hcgrid_last_error(const hcgrid_ctx* ctx);  /* ctx may be NULL (create errors) */
+
+/* ---- introspection of the pre-ordering (tests; Fig. 3, 120-124) --------
+ * Valid after a successful hcgrid_grid and a stream synchronise.  All outputs are HOST
+ * arrays; pass NULL to skip one.  Sizes come from hcgrid_get_stats (n_kept, n_rings).
+ *   sorted_pixel [n_kept]  HEALPix RING pixel index P' of every kept sample, in S' order
+ *   sorted_index [n_kept]  original sample index n of every kept sample (the "value" of
+ *                          the key-value sort)
+ *   ring_first   [1]       HEALPix ring number (1 = northernmost) of ring-table entry 0
+ *   ring_start   [n_rings+1] R_start: position in S' of the first sample of each ring;
+ *                          ring i occupies [ring_start[i], ring_start[i+1]) (0-based form
+ *                          of PAPER.md:137) */
+int hcgrid_debug_preorder(hcgrid_ctx* ctx, int64_t* sorted_pixel, int64_t* sorted_index,
+                          int32_t* ring_first, int64_t* ring_start);
+/* HEALPix RING pixel index of n points (DEVICE in, DEVICE out [n] int64): the a2 step
+ * alone, for the pixelisation self-consistency tests. */
+int hcgrid_debug_ang2pix_ring(int64_t nside, int64_t n, const double* lon_deg,
+                              const double* lat_deg, int64_t* pix, void* stream);
+
+/* The same a2 code compiled for the host: HOST in, HOST out, no GPU needed (CPU tests of
+ * the pixelisation's self-consistency). */
+int hcgrid_host_ang2pix_ring(int64_t nside, int64_t n, const double* lon_deg,
+                             const double* lat_deg, int64_t* pix);
+/* Geometry of HEALPix ring `iring` (1 = northernmost .. 4*nside-1), HOST outputs, any may
+ * be NULL: index of its first pixel, pixels in the ring, latitude of the ring centre,
+ * longitude of the centre of its pixel 0 (pixel j is centred at lon0 + j*360/npix). */
+int hcgrid_host_ring_info(int64_t nside, int32_t iring, int64_t* first_pixel, int32_t* npix,
+                          double* lat_deg, double* lon0_deg);
+
+/* Issue-rate probes for the roofline ("the builder must measure P_fp32 and
+ * P_mufu on the box"): register-only chains, 8 independent per thread, all SMs.  HOST
+ * outputs: FP32-pipe thread-instructions/s (FFMA) and MUFU.EX2 thread-instructions/s.
+ * Synchronises the device. */
+int hcgrid_measure_peaks(int device, double* fp32_inst_per_s, double* mufu_per_s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HCGRID_H */

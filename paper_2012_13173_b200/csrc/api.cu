@@ -1,0 +1,237 @@
+// api.cu -- the C-ABI of include/hcgrid.h: argument checking, context life cycle, stage
+// sequencing.  No arithmetic of the method lives here.
+#include <cmath>
+#include <cstdarg>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "hcg_common.cuh"
+
+namespace hcg {
+
+static thread_local std::string g_create_err;
+
+int fail(hcgrid_ctx* c, int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (c) c->err = buf; else g_create_err = buf;
+    return code;
+}
+
+int cuda_fail(hcgrid_ctx* c, cudaError_t e, const char* what) {
+    cudaGetLastError();   // clear the sticky-less error state
+    const int code = e == cudaErrorMemoryAllocation ? HCGRID_ERR_ALLOC : HCGRID_ERR_CUDA;
+    return fail(c, code, "CUDA error %d (%s) in %s", (int)e, cudaGetErrorString(e), what);
+}
+
+static bool is_pow2(int64_t x) { return x > 0 && (x & (x - 1)) == 0; }
+
+}  // namespace hcg
+
+using namespace hcg;
+
+extern "C" {
+
+int hcgrid_create(hcgrid_ctx** out, double sigma_deg, double support_radius_deg, int64_t nside,
+                  int precision, int device) {
+    if (!out) return fail(nullptr, HCGRID_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (!(sigma_deg > 0.0) || !std::isfinite(sigma_deg))
+        return fail(nullptr, HCGRID_ERR_INVALID_ARG, "sigma_deg must be a positive finite number");
+    if (!(support_radius_deg > 0.0) || !(support_radius_deg < 90.0))
+        return fail(nullptr, HCGRID_ERR_INVALID_ARG, "support_radius_deg must be in (0, 90)");
+    if (!is_pow2(nside) || nside > 8192)
+        return fail(nullptr, HCGRID_ERR_INVALID_ARG, "nside must be a power of two in [1, 8192]");
+    if (precision != HCGRID_F32 && precision != HCGRID_F64)
+        return fail(nullptr, HCGRID_ERR_INVALID_ARG, "precision must be HCGRID_F32 or HCGRID_F64");
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaGetDeviceCount");
+    if (device < 0 || device >= ndev)
+        return fail(nullptr, HCGRID_ERR_INVALID_ARG, "device %d out of range (%d devices)", device, ndev);
+    hcgrid_ctx* c = new (std::nothrow) hcgrid_ctx();
+    if (!c) return fail(nullptr, HCGRID_ERR_ALLOC, "out of host memory");
+    c->device = device;
+    c->precision = precision;
+    c->nside = (int)nside;
+    e = cudaSetDevice(device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, device);
+    if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "device set-up"); }
+    for (auto& ev : c->ev) {
+        e = cudaEventCreate(&ev);
+        if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaEventCreate"); }
+    }
+    KernelParams& kp = c->kp;
+    kp.sigma = sigma_deg * kDeg2Rad;
+    kp.radius = support_radius_deg * kDeg2Rad;
+    kp.inv2s2 = 1.0 / (2.0 * kp.sigma * kp.sigma);
+    const double sr = std::sin(0.5 * kp.radius);
+    kp.hav_max = sr * sr;
+    kp.h4max = (float)(4.0 * sr * sr);
+    const double log2e = 1.4426950408889634074;
+    kp.k1 = (float)(-log2e * kp.inv2s2);
+    kp.k2 = (float)(-log2e * kp.inv2s2 / 12.0);
+    *out = c;
+    return HCGRID_OK;
+}
+
+int hcgrid_destroy(hcgrid_ctx* c) {
+    if (!c) return HCGRID_OK;
+    cudaSetDevice(c->device);
+    DevBuf* bufs[] = {&c->d_strips, &c->d_wins, &c->d_cell_lon, &c->d_cell_lat, &c->d_keys, &c->d_keys_out,
+                      &c->d_idx, &c->d_idx_out, &c->d_sort_tmp, &c->d_bins, &c->d_rec, &c->d_misc,
+                      &c->d_in_lon, &c->d_in_lat, &c->d_in_val, &c->d_in_wgt, &c->d_out_cube, &c->d_out_w,
+                      &c->d_out_cnt};
+    for (DevBuf* b : bufs) b->release();
+    for (auto& ev : c->ev) if (ev) cudaEventDestroy(ev);
+    delete c;
+    return HCGRID_OK;
+}
+
+int hcgrid_set_option(hcgrid_ctx* c, int option, int64_t value) {
+    if (!c) return HCGRID_ERR_INVALID_ARG;
+    switch (option) {
+        case HCGRID_OPT_PROFILE: c->opt_profile = value != 0; break;
+        case HCGRID_OPT_SUBPIX_BITS:
+            if (value < -1 || value > 6) return fail(c, HCGRID_ERR_INVALID_ARG, "subpix bits must be -1 (auto) or 0..6");
+            c->opt_subpix = value < 0 ? -1000 : (int)value;
+            break;
+        case HCGRID_OPT_COARSEN:
+            if (value < 0 || value > 8) return fail(c, HCGRID_ERR_INVALID_ARG, "coarsen must be 0 (auto) or 1..8");
+            c->opt_coarsen = (int)value;
+            break;
+        case HCGRID_OPT_KERNEL:
+            if (value < 0 || value > 3) return fail(c, HCGRID_ERR_INVALID_ARG, "kernel must be 0..3");
+            c->opt_kernel = (int)value;
+            break;
+        case HCGRID_OPT_WARPS_PER_SM:
+            if (value < 0 || value > 64) return fail(c, HCGRID_ERR_INVALID_ARG, "warps per SM must be 0..64");
+            c->opt_warps = (int)value;
+            break;
+        default: return fail(c, HCGRID_ERR_INVALID_ARG, "unknown option %d", option);
+    }
+    return HCGRID_OK;
+}
+
+int hcgrid_set_target_car(hcgrid_ctx* c, int32_t nx, int32_t ny, double lon0, double lat0, double dlon,
+                          double dlat) {
+    if (!c) return HCGRID_ERR_INVALID_ARG;
+    if (nx < 1 || ny < 1 || (int64_t)nx * ny > (int64_t)1 << 30)
+        return fail(c, HCGRID_ERR_INVALID_ARG, "nx, ny must be >= 1 and nx*ny <= 2^30");
+    if (!std::isfinite(lon0) || !std::isfinite(lat0) || !std::isfinite(dlon) || !std::isfinite(dlat) ||
+        dlon == 0.0 || dlat == 0.0)
+        return fail(c, HCGRID_ERR_INVALID_ARG, "lon0, lat0 finite and dlon, dlat finite non-zero required");
+    if (std::fabs(dlon) * (nx - 1) >= 360.0)
+        return fail(c, HCGRID_ERR_INVALID_ARG, "a target row must span less than 360 degrees");
+    HCG_CUDA(c, cudaSetDevice(c->device));
+    c->has_target = false;
+    return build_target_car(c, nx, ny, lon0, lat0, dlon, dlat);
+}
+
+int hcgrid_set_target_cells(hcgrid_ctx* c, int64_t ncell, const double* lon, const double* lat, void* stream) {
+    if (!c) return HCGRID_ERR_INVALID_ARG;
+    if (ncell < 1 || ncell > (int64_t)1 << 26)
+        return fail(c, HCGRID_ERR_INVALID_ARG, "ncell must be in [1, 2^26] for an arbitrary-cell target");
+    if (!lon || !lat) return fail(c, HCGRID_ERR_INVALID_ARG, "lon_deg / lat_deg is NULL");
+    HCG_CUDA(c, cudaSetDevice(c->device));
+    c->has_target = false;
+    return build_target_cells(c, ncell, lon, lat, (cudaStream_t)stream);
+}
+
+int hcgrid_grid(hcgrid_ctx* c, int64_t n, const double* lon, const double* lat, const float* values,
+                int32_t nchan, const float* weights, void* cube, void* wmap, int32_t* counts, void* stream) {
+    if (!c) return HCGRID_ERR_INVALID_ARG;
+    if (!c->has_target) return fail(c, HCGRID_ERR_NO_TARGET, "no target set (call hcgrid_set_target_* first)");
+    if (n < 0 || n > 2000000000LL) return fail(c, HCGRID_ERR_INVALID_ARG, "n must be in [0, 2e9]");
+    if (nchan < 1) return fail(c, HCGRID_ERR_INVALID_ARG, "nchan must be >= 1");
+    if (n > 0 && (!lon || !lat || !values)) return fail(c, HCGRID_ERR_INVALID_ARG, "lon/lat/values is NULL");
+    if (!cube || !wmap) return fail(c, HCGRID_ERR_INVALID_ARG, "datacube / weightmap is NULL");
+    HCG_CUDA(c, cudaSetDevice(c->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    c->last_lon = lon; c->last_lat = lat; c->last_n = n; c->last_stream = st;
+    c->ev_valid = false;
+    c->stats = hcgrid_stats{};
+    c->stats.n_samples = n;
+    int rc = run_preorder(c, n, lon, lat, values, nchan, weights, st);
+    if (rc != HCGRID_OK) return rc;
+    rc = run_convolve(c, n, values, nchan, weights != nullptr, cube, wmap, counts, st);
+    if (rc != HCGRID_OK) return rc;
+    if (c->opt_profile) { cudaEventRecord(c->ev[5], st); c->ev_valid = true; }
+    c->stats.n_kept = -1;   // resolved lazily by hcgrid_get_stats
+    return HCGRID_OK;
+}
+
+int hcgrid_grid_host(hcgrid_ctx* c, int64_t n, const double* lon, const double* lat, const float* values,
+                     int32_t nchan, const float* weights, void* cube, void* wmap, int32_t* counts) {
+    if (!c) return HCGRID_ERR_INVALID_ARG;
+    if (!c->has_target) return fail(c, HCGRID_ERR_NO_TARGET, "no target set (call hcgrid_set_target_* first)");
+    if (n < 0 || nchan < 1) return fail(c, HCGRID_ERR_INVALID_ARG, "n >= 0 and nchan >= 1 required");
+    if (n > 0 && (!lon || !lat || !values)) return fail(c, HCGRID_ERR_INVALID_ARG, "lon/lat/values is NULL");
+    if (!cube || !wmap) return fail(c, HCGRID_ERR_INVALID_ARG, "datacube / weightmap is NULL");
+    HCG_CUDA(c, cudaSetDevice(c->device));
+    const size_t nn = (size_t)n, nc = (size_t)c->ncell;
+    const size_t osz = c->precision == HCGRID_F64 ? 8 : 4;
+    HCG_CUDA(c, c->d_in_lon.ensure(nn * 8 + 8));
+    HCG_CUDA(c, c->d_in_lat.ensure(nn * 8 + 8));
+    HCG_CUDA(c, c->d_in_val.ensure(nn * (size_t)nchan * 4 + 16));
+    if (weights) HCG_CUDA(c, c->d_in_wgt.ensure(nn * 4 + 16));
+    HCG_CUDA(c, c->d_out_cube.ensure(nc * (size_t)nchan * osz));
+    HCG_CUDA(c, c->d_out_w.ensure(nc * osz));
+    if (counts) HCG_CUDA(c, c->d_out_cnt.ensure(nc * 4));
+    cudaStream_t st = nullptr;   // legacy default stream: ordered with everything
+    if (n > 0) {
+        HCG_CUDA(c, cudaMemcpyAsync(c->d_in_lon.p, lon, nn * 8, cudaMemcpyHostToDevice, st));
+        HCG_CUDA(c, cudaMemcpyAsync(c->d_in_lat.p, lat, nn * 8, cudaMemcpyHostToDevice, st));
+        HCG_CUDA(c, cudaMemcpyAsync(c->d_in_val.p, values, nn * (size_t)nchan * 4, cudaMemcpyHostToDevice, st));
+        if (weights) HCG_CUDA(c, cudaMemcpyAsync(c->d_in_wgt.p, weights, nn * 4, cudaMemcpyHostToDevice, st));
+    }
+    const int rc = hcgrid_grid(c, n, c->d_in_lon.as<double>(), c->d_in_lat.as<double>(), c->d_in_val.as<float>(),
+                               nchan, weights ? c->d_in_wgt.as<float>() : nullptr, c->d_out_cube.p, c->d_out_w.p,
+                               counts ? c->d_out_cnt.as<int32_t>() : nullptr, st);
+    if (rc != HCGRID_OK) return rc;
+    HCG_CUDA(c, cudaMemcpyAsync(cube, c->d_out_cube.p, nc * (size_t)nchan * osz, cudaMemcpyDeviceToHost, st));
+    HCG_CUDA(c, cudaMemcpyAsync(wmap, c->d_out_w.p, nc * osz, cudaMemcpyDeviceToHost, st));
+    if (counts) HCG_CUDA(c, cudaMemcpyAsync(counts, c->d_out_cnt.p, nc * 4, cudaMemcpyDeviceToHost, st));
+    HCG_CUDA(c, cudaStreamSynchronize(st));
+    return HCGRID_OK;
+}
+
+int64_t hcgrid_ncell(const hcgrid_ctx* c) { return c && c->has_target ? c->ncell : 0; }
+
+int hcgrid_get_stats(const hcgrid_ctx* cc, hcgrid_stats* out) {
+    hcgrid_ctx* c = const_cast<hcgrid_ctx*>(cc);
+    if (!c || !out) return HCGRID_ERR_INVALID_ARG;
+    HCG_CUDA(c, cudaSetDevice(c->device));
+    if (c->stats.n_kept < 0) {
+        HCG_CUDA(c, cudaStreamSynchronize(c->last_stream));
+        int32_t kept = 0;
+        HCG_CUDA(c, cudaMemcpy(&kept, c->d_bins.as<int32_t>() + c->region.nbins, 4, cudaMemcpyDeviceToHost));
+        c->stats.n_kept = kept;
+    }
+    if (c->ev_valid) {
+        HCG_CUDA(c, cudaEventSynchronize(c->ev[5]));
+        float* dst[5] = {&c->stats.us_pixelise, &c->stats.us_sort, &c->stats.us_tables, &c->stats.us_pack,
+                         &c->stats.us_convolve};
+        for (int i = 0; i < 5; ++i) {
+            float ms = 0.f;
+            HCG_CUDA(c, cudaEventElapsedTime(&ms, c->ev[i], c->ev[i + 1]));
+            *dst[i] = ms * 1000.f;
+        }
+        float ms = 0.f;
+        HCG_CUDA(c, cudaEventElapsedTime(&ms, c->ev[0], c->ev[5]));
+        c->stats.us_total = ms * 1000.f;
+    }
+    c->stats.n_bins = c->region.nbins;
+    c->stats.n_rings = c->region.nring;
+    c->stats.subpix_bits = c->region.subpix;
+    *out = c->stats;
+    return HCGRID_OK;
+}
+
+const char* hcgrid_last_error(const hcgrid_ctx* c) { return c ? c->err.c_str() : g_create_err.c_str(); }
+
+}  // extern "C"

@@ -1,0 +1,328 @@
+// convolve.cu -- step a6: the gather-style convolution (Sect. 3.4 i-v;
+// Eq. 1; kernel PAPER.md:186), hand-written for sm_100a.
+//
+// Organisation: one WARP owns a task = G consecutive cells of a strip
+// (the paper's thread coarsening, at warp scope) and its 32 lanes stride
+// over the candidate samples, so every load is a contiguous slice of S' and every cell
+// gets 32 partial sums that are combined with shuffles -- no atomics anywhere.
+//   step (i)   ring range of the disc: the strip's precomputed RingWin row (a1)
+//   step (ii)  per ring, lane k turns the disc's longitude extent into a bin range
+//   step (iii) two per-pixel-table reads give the sample range [S_start, S_end)
+//   step (iv)  the ranges of all rings are concatenated into one candidate stream; in the
+//              staged kernel each lane issues ONE bulk async copy (cp.async.bulk, the
+//              TMA engine) of its ring's slice into the warp's shared-memory buffer, so
+//              the stream is flattened by the copy engine, double-buffered on mbarriers
+//   step (v)   pair arithmetic on exact fixed-point coordinate differences in fp32.
+#include <cstdarg>
+#include <cstring>
+
+#include "hcg_conv.cuh"
+
+namespace hcg {
+
+template <int G>
+struct Acc32 {
+    float W[G], S[G];
+    int cnt[G];
+};
+
+// Step (v) for one candidate against the G cells of the task.  Coordinates: exact integer
+// differences of the fixed-point positions -> fp32 radians; 4 hav(d) from the small-angle
+// series h4 = u(1-u/12) + cos(phi_c)cos(phi_s) v(1-v/12), u = dphi^2, v = dlam^2; accept
+// iff h4 <= 4 sin^2(R/2); d^2 = h4(1+h4/12); w = 2^(-d^2 log2e / 2 sigma^2).
+template <int G, bool HASQ>
+__device__ __forceinline__ void pair_update(const Rec32& r, const TaskConst& tc, Acc32<G>& acc) {
+    const float dx0 = (float)(int)(r.xi - tc.xc0) * tc.qx;
+    const float dy = (float)(int)(r.yi - tc.yc) * tc.qy;
+    const float u = dy * dy;
+    const float u2 = u * fmaf(u, -1.0f / 12.0f, 1.0f);
+    const float C = fmaf(dy, fmaf(dy, fmaf(dy, tc.c3, tc.c2), tc.c1), tc.c0);
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+        const float dx = fmaf((float)g, -tc.du, dx0);
+        const float v = dx * dx;
+        const float B = v * fmaf(v, -1.0f / 12.0f, 1.0f);
+        const float h4 = fmaf(C, B, u2);
+        const float e = h4 * fmaf(h4, tc.k2, tc.k1);
+        float w = ex2_approx(e);
+        if (HASQ) w *= r.q;
+        if (h4 <= tc.h4max) {
+            acc.W[g] += w;
+            acc.S[g] = fmaf(w, r.v, acc.S[g]);
+            acc.cnt[g] += 1;
+        }
+    }
+}
+
+template <int G>
+__device__ __forceinline__ void task_finish(Acc32<G>& acc, int lane, int64_t cell0, int ncells,
+                                            float* __restrict__ cube, float* __restrict__ wmap,
+                                            int32_t* __restrict__ counts) {
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            acc.W[g] += __shfl_xor_sync(0xffffffffu, acc.W[g], o);
+            acc.S[g] += __shfl_xor_sync(0xffffffffu, acc.S[g], o);
+            acc.cnt[g] += __shfl_xor_sync(0xffffffffu, acc.cnt[g], o);
+        }
+    }
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+        if (lane == g && g < ncells) {
+            const float W = acc.W[g];
+            cube[cell0 + g] = W > 0.0f ? acc.S[g] / W : __int_as_float(0x7fc00000);
+            wmap[cell0 + g] = W;
+            if (counts) counts[cell0 + g] = acc.cnt[g];
+        }
+    }
+}
+
+// ------------------------------------------------------------------ kernel A: simple
+// Warp per task, candidates read straight from global memory ring by ring.  Kept as the
+// plainly-correct reference organisation (HCGRID_OPT_KERNEL = 1) and for kmax > 32.
+template <int G, bool HASQ>
+__global__ void __launch_bounds__(256)
+conv1_simple_f32(const ConvArgs a) {
+    const int lane = threadIdx.x & 31;
+    const int64_t task = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (task >= a.ntasks) return;
+    const int s = (int)(task / a.tasks_per_strip);
+    const int ix0 = (int)(task % a.tasks_per_strip) * G;
+    const int ncells = min(G, a.strip_cells - ix0);
+    const Strip st = a.strips[s];
+    const TaskConst tc = make_task_const(a, st, ix0);
+    const Rec32* __restrict__ rec = (const Rec32*)a.rec;
+    Acc32<G> acc;
+#pragma unroll
+    for (int g = 0; g < G; ++g) { acc.W[g] = 0.f; acc.S[g] = 0.f; acc.cnt[g] = 0; }
+    for (int k = 0; k < st.nring; ++k) {
+        const RingWin w = a.wins[(size_t)s * a.kmax + k];
+        int sa, sn;
+        ring_segment(w, ix0, ncells, a.rg, a.bin_start, sa, sn);
+        for (int i = lane; i < sn; i += 32) {
+            const uint4 raw = __ldg((const uint4*)(rec + sa + i));
+            Rec32 r;
+            r.xi = raw.x; r.yi = raw.y; r.idx = raw.z; r.q = __uint_as_float(raw.w);
+            pair_update<G, HASQ>(r, tc, acc);
+        }
+    }
+    task_finish<G>(acc, lane, (int64_t)s * a.strip_cells + ix0, ncells, (float*)a.cube, (float*)a.wmap, a.counts);
+}
+
+// ------------------------------------------------------------------ kernel B: staged (TMA)
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "W_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra D_%=;\n\t"
+        "bra W_%=;\n\t"
+        "D_%=:\n\t}" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+
+// Persistent warps; each warp walks tasks  warp_id, warp_id + nwarps, ...  Every task is a
+// stream of `total` candidates cut into chunks of a.chunk records; chunk j+1 (possibly the
+// first chunk of the NEXT task) is in flight while chunk j is computed.
+template <int G, bool HASQ>
+__global__ void __launch_bounds__(128)
+conv1_staged_f32(const ConvArgs a) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int lane = threadIdx.x & 31;
+    const int wib = threadIdx.x >> 5;
+    const int nwib = blockDim.x >> 5;
+    const int64_t nwarps = (int64_t)gridDim.x * nwib;
+    const int64_t warp_id = (int64_t)blockIdx.x * nwib + wib;
+    const int CH = a.chunk;
+    Rec32* buf0 = (Rec32*)(smem + (size_t)wib * 2 * CH * sizeof(Rec32));
+    Rec32* buf1 = buf0 + CH;
+    uint64_t* bars = (uint64_t*)(smem + (size_t)nwib * 2 * CH * sizeof(Rec32)) + wib * 2;
+    const uint32_t bar0 = smem_u32(bars), bar1 = smem_u32(bars + 1);
+    if (lane == 0) {
+        mbar_init(bar0, 1);
+        mbar_init(bar1, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+    const Rec32* __restrict__ rec = (const Rec32*)a.rec;
+
+    // per-lane segment state of a task: lane k owns ring k of the strip's table row
+    struct Segs { int a, n, p, total; int s, ix0, ncells; };
+    auto prepare = [&](int64_t task, Segs& sg) {
+        sg.s = (int)(task / a.tasks_per_strip);
+        sg.ix0 = (int)(task % a.tasks_per_strip) * G;
+        sg.ncells = min(G, a.strip_cells - sg.ix0);
+        const int nring = a.strips[sg.s].nring;
+        sg.a = 0; sg.n = 0;
+        if (lane < nring) {
+            const RingWin w = a.wins[(size_t)sg.s * a.kmax + lane];
+            ring_segment(w, sg.ix0, sg.ncells, a.rg, a.bin_start, sg.a, sg.n);
+        }
+        int incl = sg.n;                       // inclusive prefix sum over lanes
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += t;
+        }
+        sg.p = incl - sg.n;
+        sg.total = __shfl_sync(0xffffffffu, incl, 31);
+    };
+    auto issue = [&](const Segs& sg, int chunk, Rec32* buf, uint32_t bar) {
+        const int c0 = chunk * CH;
+        const int c1 = min(c0 + CH, sg.total);
+        const int lo = max(sg.p, c0), hi = min(sg.p + sg.n, c1);
+        if (lane == 0) mbar_expect_tx(bar, (uint32_t)(c1 - c0) * (uint32_t)sizeof(Rec32));
+        __syncwarp();
+        if (hi > lo)
+            bulk_g2s(smem_u32(buf + (lo - c0)), rec + sg.a + (lo - sg.p), (uint32_t)(hi - lo) * (uint32_t)sizeof(Rec32), bar);
+    };
+
+    int64_t task = warp_id;
+    if (task >= a.ntasks) return;
+    Segs cur, nxt;
+    prepare(task, cur);
+    int chunk = 0;                 // chunk of `cur` that sits (or is arriving) in buffer `b`
+    int b = 0;
+    uint32_t ph0 = 0, ph1 = 0;     // phase parity of the two barriers
+    if (cur.total > 0) issue(cur, 0, buf0, bar0);
+    Acc32<G> acc;
+#pragma unroll
+    for (int g = 0; g < G; ++g) { acc.W[g] = 0.f; acc.S[g] = 0.f; acc.cnt[g] = 0; }
+    TaskConst tc = make_task_const(a, a.strips[cur.s], cur.ix0);
+
+    while (true) {
+        const int nchunks = (cur.total + CH - 1) / CH;
+        const bool have_chunk = chunk < nchunks;
+        const bool last = chunk + 1 >= nchunks;
+        // the chunk that follows goes to the other buffer (or to this one if it is unused)
+        const int nb = have_chunk ? (b ^ 1) : b;
+        bool have_next_task = false;
+        if (!last) {
+            issue(cur, chunk + 1, nb ? buf1 : buf0, nb ? bar1 : bar0);
+        } else {
+            const int64_t t2 = task + nwarps;
+            if (t2 < a.ntasks) {
+                have_next_task = true;
+                prepare(t2, nxt);                  // empty tasks still have outputs to write
+                if (nxt.total > 0) issue(nxt, 0, nb ? buf1 : buf0, nb ? bar1 : bar0);
+            }
+        }
+        if (have_chunk) {
+            const Rec32* buf = b ? buf1 : buf0;
+            mbar_wait(b ? bar1 : bar0, b ? ph1 : ph0);
+            if (b) ph1 ^= 1; else ph0 ^= 1;
+            const int cnt = min(CH, cur.total - chunk * CH);
+            for (int i = lane; i < cnt; i += 32) {
+                const uint4 raw = *(const uint4*)(buf + i);
+                Rec32 r;
+                r.xi = raw.x; r.yi = raw.y; r.idx = raw.z; r.q = __uint_as_float(raw.w);
+                pair_update<G, HASQ>(r, tc, acc);
+            }
+            __syncwarp();
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        }
+        b = nb;
+        if (!last) { ++chunk; continue; }
+        task_finish<G>(acc, lane, (int64_t)cur.s * a.strip_cells + cur.ix0, cur.ncells,
+                       (float*)a.cube, (float*)a.wmap, a.counts);
+        if (!have_next_task) break;
+        task += nwarps;
+        cur = nxt;
+        chunk = 0;
+#pragma unroll
+        for (int g = 0; g < G; ++g) { acc.W[g] = 0.f; acc.S[g] = 0.f; acc.cnt[g] = 0; }
+        tc = make_task_const(a, a.strips[cur.s], cur.ix0);
+    }
+}
+
+
+// ------------------------------------------------------------------ launcher
+template <int G>
+static int launch_f32(hcgrid_ctx* c, ConvArgs& a, bool hasq, bool staged, cudaStream_t st) {
+    a.coarsen = G;
+    a.tasks_per_strip = (a.strip_cells + G - 1) / G;
+    a.ntasks = (int64_t)a.tasks_per_strip * c->nstrip;
+    if (a.ntasks == 0) return HCGRID_OK;
+    if (!staged) {
+        const unsigned blocks = (unsigned)((a.ntasks + 7) / 8);
+        if (hasq) conv1_simple_f32<G, true><<<blocks, 256, 0, st>>>(a);
+        else conv1_simple_f32<G, false><<<blocks, 256, 0, st>>>(a);
+    } else {
+        const int wpb = 4;
+        const int warps_sm = c->opt_warps > 0 ? c->opt_warps : 32;
+        const int blocks_sm = (warps_sm + wpb - 1) / wpb;
+        // two staging buffers per warp, sized so blocks_sm blocks fit the SM's shared memory
+        int chunk = (int)((200 * 1024 / blocks_sm - 64) / (wpb * 2 * sizeof(Rec32)));
+        chunk = chunk > 512 ? 512 : chunk & ~31;
+        if (chunk < 32) chunk = 32;
+        a.chunk = chunk;
+        const size_t smem = (size_t)wpb * 2 * chunk * sizeof(Rec32) + wpb * 2 * sizeof(uint64_t);
+        int64_t blocks = (int64_t)blocks_sm * c->num_sms;
+        const int64_t need = (a.ntasks + wpb - 1) / wpb;
+        if (blocks > need) blocks = need;
+        auto k = hasq ? conv1_staged_f32<G, true> : conv1_staged_f32<G, false>;
+        HCG_CUDA(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        k<<<(unsigned)blocks, wpb * 32, smem, st>>>(a);
+    }
+    HCG_CUDA(c, cudaGetLastError());
+    return HCGRID_OK;
+}
+
+int run_convolve(hcgrid_ctx* c, int64_t n, const float* values, int nchan, bool has_weights, void* cube,
+                 void* wmap, int32_t* counts, cudaStream_t st) {
+    (void)n;
+    const Region& rg = c->region;
+    ConvArgs a{};
+    a.strips = c->d_strips.as<Strip>();
+    a.wins = c->d_wins.as<RingWin>();
+    a.bin_start = c->d_bins.as<int32_t>();
+    a.rec = c->d_rec.p;
+    a.values = values;
+    a.cube = cube; a.wmap = wmap; a.counts = counts;
+    a.rg = rg; a.kp = c->kp;
+    a.kmax = c->kmax; a.strip_cells = c->strip_cells;
+    a.nchan = nchan;
+    a.qx = (float)(rg.wx / 4294967296.0);
+    a.qy = (float)(rg.wy / 4294967296.0);
+    a.sx = 4294967296.0 / rg.wx;
+    const bool f32 = c->precision == HCGRID_F32 && c->f32_series_ok && c->opt_kernel != 2;
+    int rc;
+    if (f32 && nchan == 1 && c->opt_kernel != 3) {
+        const bool staged = c->opt_kernel != 1 && c->kmax <= 32;
+        int G = c->opt_coarsen;
+        if (G == 0) G = c->strip_cells >= 4 ? 2 : 1;
+        if (G > c->strip_cells) G = 1;
+        switch (G) {
+            case 1: rc = launch_f32<1>(c, a, has_weights, staged, st); break;
+            case 2: rc = launch_f32<2>(c, a, has_weights, staged, st); break;
+            case 3: rc = launch_f32<3>(c, a, has_weights, staged, st); break;
+            case 4: rc = launch_f32<4>(c, a, has_weights, staged, st); break;
+            case 6: rc = launch_f32<6>(c, a, has_weights, staged, st); break;
+            case 8: rc = launch_f32<8>(c, a, has_weights, staged, st); break;
+            default: return fail(c, HCGRID_ERR_INVALID_ARG, "coarsen %d not built (1,2,3,4,6,8)", G);
+        }
+        c->stats.coarsen = G;
+        c->stats.kernel = staged ? 2 : 1;
+    } else {
+        rc = launch_conv_general(c, a, !f32, c->precision == HCGRID_F64, st);
+        c->stats.coarsen = 1;
+        c->stats.kernel = f32 ? 3 : (c->precision == HCGRID_F64 ? 5 : 4);
+    }
+    if (rc == HCGRID_OK) c->stats.gpu_launches += 1;
+    return rc;
+}
+
+}  // namespace hcg

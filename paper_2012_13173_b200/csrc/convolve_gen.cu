@@ -1,0 +1,184 @@
+// convolve_gen.cu -- step a6, the general kernel: any channel count, fp32 or fp64 pair
+// arithmetic, fp32 or fp64 accumulation (Sect. 3.4 i-v; Eq. 1).
+//
+// One warp owns one cell.  Phase 1: the 32 lanes evaluate 32 consecutive candidates of the
+// cell's ring windows (distance test + kernel weight).  Phase 2 (nchan > 1): the accepted
+// candidates of the batch are visited one by one and the whole warp reads that sample's
+// spectrum row in place (values[idx][*], contiguous, coalesced) -- lane l owns channels
+// 4l..4l+3 and 128+4l..128+4l+3 of a 256-channel tile -- so every channel has one register
+// accumulator and Eq. 1's "same weight for all channels" costs one FMA per
+// channel per accepted pair.  The spectra are never moved (a5: values stay in input order).
+//
+// fp64 pair arithmetic follows the definition with no shortcut: differences formed in
+// degrees first, haversine, d = 2 asin(sqrt(hav)), w = exp(-d^2/(2 sigma^2)).
+#include "hcg_conv.cuh"
+
+namespace hcg {
+
+template <typename T> struct NanOf;
+template <> struct NanOf<float> { static __device__ float v() { return __int_as_float(0x7fc00000); } };
+template <> struct NanOf<double> { static __device__ double v() { return __longlong_as_double(0x7ff8000000000000LL); } };
+
+template <typename T>
+__device__ __forceinline__ T warp_sum(T x) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    return x;
+}
+
+// fp64 pair: returns hit; w = q-less kernel weight
+__device__ __forceinline__ bool pair64(const Rec64& r, double clon_deg, double clat_deg, double ccos,
+                                       const KernelParams& kp, double& w) {
+    const double dlat = (r.lat_deg - clat_deg) * kDeg2Rad;
+    const double dlon = remainder(r.lon_deg - clon_deg, 360.0) * kDeg2Rad;
+    const double sa = sin(0.5 * dlat), sb = sin(0.5 * dlon);
+    double hav = sa * sa + ccos * r.coslat * sb * sb;
+    if (hav > 1.0) hav = 1.0;
+    const double d = 2.0 * asin(sqrt(hav));
+    w = exp(-d * d * kp.inv2s2);
+    return d <= kp.radius;
+}
+
+template <bool PAIR64, typename AccT, bool VEC4>
+__global__ void __launch_bounds__(256)
+conv_general(const ConvArgs a) {
+    const int lane = threadIdx.x & 31;
+    const int64_t task = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (task >= a.ntasks) return;
+    const int s = (int)(task / a.strip_cells);
+    const int ix = (int)(task % a.strip_cells);
+    const Strip st = a.strips[s];
+    const int nchan = a.nchan;
+    const float* __restrict__ values = a.values;
+    AccT* __restrict__ cube = (AccT*)a.cube;
+    AccT* __restrict__ wmap = (AccT*)a.wmap;
+
+    // cell constants
+    TaskConst tc;
+    double clon_deg = 0.0, clat_deg = 0.0, ccos = 0.0;
+    if (PAIR64) {
+        clon_deg = __dadd_rn(st.lon0_deg, __dmul_rn((double)ix, st.dlon_deg));   // no FMA (SURVEY 8c fp64 pin)
+        clat_deg = st.lat_deg;
+        ccos = cos(clat_deg * kDeg2Rad);
+    } else {
+        tc = make_task_const(a, st, ix);
+    }
+
+    for (int ch0 = 0; ch0 < nchan; ch0 += 256) {
+        AccT acc[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) acc[j] = (AccT)0;
+        AccT W = (AccT)0;
+        int cnt = 0;
+        for (int k = 0; k < st.nring; ++k) {
+            const RingWin w = a.wins[(size_t)s * a.kmax + k];
+            int sa, sn;
+            ring_segment(w, ix, 1, a.rg, a.bin_start, sa, sn);
+            for (int base = 0; base < sn; base += 32) {
+                const int i = base + lane;
+                bool hit = false;
+                AccT wq = (AccT)0;
+                uint32_t idx = 0;
+                if (i < sn) {
+                    if (PAIR64) {
+                        const Rec64 r = ((const Rec64*)a.rec)[sa + i];
+                        double wd;
+                        hit = pair64(r, clon_deg, clat_deg, ccos, a.kp, wd);
+                        wq = (AccT)(wd * (double)r.q);
+                        idx = r.idx;
+                    } else {
+                        const uint4 raw = __ldg((const uint4*)a.rec + sa + i);
+                        Rec32 r;
+                        r.xi = raw.x; r.yi = raw.y; r.idx = raw.z; r.q = __uint_as_float(raw.w);
+                        float wf;
+                        hit = pair32(r, tc, wf);
+                        wq = (AccT)(wf * r.q);
+                        idx = r.idx;
+                    }
+                }
+                if (hit) { W += wq; cnt += 1; }
+                if (nchan == 1) {
+                    if (hit) acc[0] += wq * (AccT)(PAIR64 ? __ldg(values + idx) : __uint_as_float(idx));
+                } else {
+                    unsigned m = __ballot_sync(0xffffffffu, hit);
+                    while (m) {
+                        const int b = __ffs(m) - 1;
+                        m &= m - 1;
+                        const AccT wb = __shfl_sync(0xffffffffu, wq, b);
+                        const uint32_t ib = __shfl_sync(0xffffffffu, idx, b);
+                        const float* __restrict__ row = values + (size_t)ib * nchan + ch0;
+                        if (VEC4) {
+#pragma unroll
+                            for (int j = 0; j < 2; ++j) {
+                                const int c = 4 * lane + 128 * j;
+                                if (ch0 + c < nchan) {
+                                    const float4 v = __ldg((const float4*)(row + c));
+                                    acc[4 * j + 0] += wb * (AccT)v.x;
+                                    acc[4 * j + 1] += wb * (AccT)v.y;
+                                    acc[4 * j + 2] += wb * (AccT)v.z;
+                                    acc[4 * j + 3] += wb * (AccT)v.w;
+                                }
+                            }
+                        } else {
+#pragma unroll
+                            for (int j = 0; j < 8; ++j) {
+                                const int c = lane + 32 * j;
+                                if (ch0 + c < nchan) acc[j] += wb * (AccT)__ldg(row + c);
+                            }
+                        }
+                    }
+                }
+            }
+        }
+        W = warp_sum(W);
+        cnt = warp_sum(cnt);
+        const AccT nan = NanOf<AccT>::v();
+        if (nchan == 1) {
+            const AccT S = warp_sum(acc[0]);
+            if (lane == 0) cube[task] = W > (AccT)0 ? S / W : nan;
+        } else if (VEC4) {
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                const int c = ch0 + 4 * lane + 128 * j;
+                if (c < nchan) {
+                    AccT* o = cube + (size_t)task * nchan + c;
+#pragma unroll
+                    for (int t = 0; t < 4; ++t) o[t] = W > (AccT)0 ? acc[4 * j + t] / W : nan;
+                }
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const int c = ch0 + lane + 32 * j;
+                if (c < nchan) cube[(size_t)task * nchan + c] = W > (AccT)0 ? acc[j] / W : nan;
+            }
+        }
+        if (ch0 == 0 && lane == 0) {
+            wmap[task] = W;
+            if (a.counts) a.counts[task] = cnt;
+        }
+    }
+}
+
+int launch_conv_general(hcgrid_ctx* c, const ConvArgs& a0, bool pair_f64, bool out_double, cudaStream_t st) {
+    ConvArgs a = a0;
+    a.ntasks = c->ncell;
+    a.tasks_per_strip = a.strip_cells;
+    const bool vec4 = (a.nchan % 4 == 0) && ((uintptr_t)a.values % 16 == 0);
+    const int threads = 256;
+    const unsigned blocks = (unsigned)((a.ntasks + 7) / 8);
+    if (blocks == 0) return HCGRID_OK;
+#define HCG_LAUNCH(P, T, V) conv_general<P, T, V><<<blocks, threads, 0, st>>>(a)
+    if (out_double) {
+        if (vec4) HCG_LAUNCH(true, double, true); else HCG_LAUNCH(true, double, false);
+    } else if (pair_f64) {
+        if (vec4) HCG_LAUNCH(true, float, true); else HCG_LAUNCH(true, float, false);
+    } else {
+        if (vec4) HCG_LAUNCH(false, float, true); else HCG_LAUNCH(false, float, false);
+    }
+#undef HCG_LAUNCH
+    HCG_CUDA(c, cudaGetLastError());
+    return HCGRID_OK;
+}
+
+}  // namespace hcg

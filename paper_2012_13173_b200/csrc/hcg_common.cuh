@@ -1,0 +1,154 @@
+// hcg_common.cuh -- shared types of libhcgrid (context, target description, device tables).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <cstdio>
+#include <string>
+
+#include "../../include/hcgrid.h"
+#include "hcg_healpix.cuh"
+
+namespace hcg {
+
+// ---------------------------------------------------------------- device-side layouts
+// One "strip" = consecutive target cells sharing a latitude with uniform longitude
+// spacing: a row of a plate-carree target, or a single cell of an arbitrary target.
+struct Strip {
+    double u0;        // (lon of cell 0 - region lon_lo) mod 2pi, rad
+    double du;        // signed lon step between cells, rad (0 for single-cell strips)
+    double lat;       // rad
+    double lon0_deg;  // lon of cell 0 in degrees as the caller gave it (fp64 kernel)
+    double dlon_deg;  // lon step in degrees
+    double lat_deg;
+    int32_t ring_lo;  // first ring (relative to region ring_first) of the strip's table
+    int32_t nring;    // entries used in the strip's table row (<= kmax)
+    uint32_t yi;      // fixed-point latitude of the strip (Rec32 convention)
+    // cos(lat_c) cos(lat_c + dy) = c0 + dy (c1 + dy (c2 + dy c3)), fp32 coefficients
+    float c0, c1, c2, c3;
+    float du_f;       // du rounded to fp32
+    int32_t pad_;
+};
+
+// Per (strip, ring) search window, precomputed by a1 (PAPER.md:136 step i-ii): the
+// lookup-bin range of the disc's longitude extent on that ring as a linear function of
+// the cell index ix along the strip.
+//   first bin = floor(a_lo + ix_west * step),  last bin = floor(a_hi + ix_east * step)
+// flags: 0 = empty (ring band does not meet the disc), 1 = window, 2 = whole ring
+struct RingWin {
+    double a_lo, a_hi, step;
+    int32_t ring_rel;
+    int32_t flags;
+    int32_t nb;       // lookup bins along this ring (whole-ring / wrap logic)
+    int32_t pad_;
+};
+
+// 16-byte packed sample S' as the fp32 convolution reads it (a5).  xi/yi are unsigned
+// fixed point over the region: lon offset u in [0, wx) -> xi = u / wx * 2^32 (wraps
+// naturally when wx = 2 pi), lat offset -> yi.  Differences of two fixed-point
+// coordinates are exact integers, which is what keeps fp32 pair arithmetic at 1e-10 rad.
+struct __align__(16) Rec32 {
+    uint32_t xi, yi;
+    union { float v; uint32_t idx; };  // value (nchan == 1) or original sample index
+    float q;                            // per-sample weight (1 if none)
+};
+
+// fp64 mode sample: caller's degrees untouched (differences are formed in degrees first)
+struct __align__(16) Rec64 {
+    double lon_deg, lat_deg;
+    double coslat;
+    uint32_t idx;
+    float q;
+};
+
+struct Region {            // what of the sphere the target can reach (host + device copy)
+    int32_t nside;
+    int32_t subpix;        // b: 2^b lookup bins per pixel (b may be negative)
+    int32_t ring_first;    // HEALPix ring number of relative ring 0
+    int32_t nring;         // rings in the tables
+    int32_t m;             // bins per ring in the table (table is [nring][m], +1 sentinel)
+    int32_t full_circle;   // 1: the longitude window is the whole circle
+    double lon_lo;         // rad, [0, 2pi)
+    double wx;             // rad, longitude extent mapped onto 2^32
+    double lat_lo;         // rad
+    double wy;             // rad, latitude extent mapped onto 2^32
+    int64_t nbins;         // nring * m
+};
+
+struct KernelParams {      // per-context constants of the pair arithmetic
+    double sigma, radius;              // rad
+    double inv2s2;                     // 1 / (2 sigma^2)
+    double hav_max;                    // sin^2(R/2)
+    float h4max;                       // 4 sin^2(R/2), rounded to fp32
+    float k1, k2;                      // exponent = h4 * (k1 + k2 * h4): -log2e/(2 sigma^2) * (1, 1/12)
+};
+
+// ---------------------------------------------------------------- host-side helpers
+struct DevBuf {
+    void* p = nullptr;
+    size_t cap = 0;
+    cudaError_t ensure(size_t bytes) {
+        if (bytes <= cap) return cudaSuccess;
+        if (p) cudaFree(p);
+        p = nullptr; cap = 0;
+        size_t want = bytes + bytes / 8 + 256;
+        cudaError_t e = cudaMalloc(&p, want);
+        if (e == cudaSuccess) cap = want;
+        return e;
+    }
+    void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+    template <class T> T* as() const { return reinterpret_cast<T*>(p); }
+};
+
+}  // namespace hcg
+
+struct hcgrid_ctx {
+    int device = 0;
+    int precision = HCGRID_F32;
+    int nside = 0;
+    int num_sms = 148;
+    hcg::KernelParams kp{};
+    // options
+    int opt_profile = 0, opt_subpix = -1000, opt_coarsen = 0, opt_kernel = 0, opt_warps = 0;
+    // target
+    bool has_target = false;
+    bool is_car = false;
+    int64_t ncell = 0;
+    int32_t nstrip = 0, strip_cells = 0, kmax = 0;
+    bool f32_series_ok = true;      // small-angle series valid over the whole target
+    double cell_width_sky = 0.0;    // min over strips of |du| cos(lat), rad (coarsening choice)
+    hcg::Region region{};
+    hcg::DevBuf d_strips, d_wins, d_cell_lon, d_cell_lat;
+    // per-call scratch
+    hcg::DevBuf d_keys, d_keys_out, d_idx, d_idx_out, d_sort_tmp, d_bins, d_rec, d_misc;
+    hcg::DevBuf d_in_lon, d_in_lat, d_in_val, d_in_wgt, d_out_cube, d_out_w, d_out_cnt;  // *_host path
+    // last call (debug introspection)
+    const double* last_lon = nullptr;
+    const double* last_lat = nullptr;
+    int64_t last_n = 0;
+    cudaStream_t last_stream = nullptr;
+    cudaEvent_t ev[8] = {};
+    bool ev_valid = false;
+    hcgrid_stats stats{};
+    std::string err;
+};
+
+namespace hcg {
+
+// stage entry points (defined in target.cu / preorder.cu / convolve*.cu)
+int build_target_car(hcgrid_ctx* c, int nx, int ny, double lon0, double lat0, double dlon, double dlat);
+int build_target_cells(hcgrid_ctx* c, int64_t ncell, const double* lon, const double* lat, cudaStream_t st);
+int run_preorder(hcgrid_ctx* c, int64_t n, const double* lon, const double* lat, const float* values,
+                 int nchan, const float* weights, cudaStream_t st);
+int run_convolve(hcgrid_ctx* c, int64_t n, const float* values, int nchan, bool has_weights,
+                 void* cube, void* wmap, int32_t* counts, cudaStream_t st);
+
+int fail(hcgrid_ctx* c, int code, const char* fmt, ...);
+int cuda_fail(hcgrid_ctx* c, cudaError_t e, const char* what);
+
+#define HCG_CUDA(c, call)                                              \
+    do {                                                               \
+        cudaError_t e_ = (call);                                       \
+        if (e_ != cudaSuccess) return hcg::cuda_fail((c), e_, #call);  \
+    } while (0)
+
+}  // namespace hcg

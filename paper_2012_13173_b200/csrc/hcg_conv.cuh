@@ -1,0 +1,94 @@
+// hcg_conv.cuh -- what the convolution kernels (convolve.cu, convolve_gen.cu) share:
+// the kernel argument block and steps (ii)+(iii) of the search.
+#pragma once
+#include "hcg_common.cuh"
+
+namespace hcg {
+
+// ------------------------------------------------------------------ shared device code
+struct ConvArgs {
+    const Strip* strips;
+    const RingWin* wins;
+    const int32_t* bin_start;
+    const void* rec;            // Rec32* or Rec64*
+    const float* values;        // original values [n][nchan] (multi-channel / fp64 kernels)
+    void* cube;
+    void* wmap;
+    int32_t* counts;
+    Region rg;
+    KernelParams kp;
+    int32_t kmax, strip_cells, tasks_per_strip, coarsen;
+    int64_t ntasks;
+    int32_t nchan;
+    int32_t chunk;              // records per staging buffer (staged kernel)
+    float qx, qy;               // radians per fixed-point unit
+    double sx;                  // fixed-point units per radian (lon)
+};
+
+__device__ __forceinline__ float ex2_approx(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// Step (ii)+(iii): sample range of ring-window `w` for the cells [ix0, ix0+g-1].
+__device__ __forceinline__ void ring_segment(const RingWin& w, int ix0, int g, const Region& rg,
+                                             const int32_t* __restrict__ bin_start, int& a, int& n) {
+    a = 0; n = 0;
+    if (w.flags == 0) return;
+    long long jlo, jhi;
+    if (w.flags == 2) {
+        jlo = 0; jhi = (w.nb < rg.m ? w.nb : rg.m) - 1;
+    } else {
+        const int ixw = w.step >= 0.0 ? ix0 : ix0 + g - 1;
+        const int ixe = w.step >= 0.0 ? ix0 + g - 1 : ix0;
+        jlo = (long long)floor(w.a_lo + (double)ixw * w.step);
+        jhi = (long long)floor(w.a_hi + (double)ixe * w.step);
+        if (rg.full_circle) {
+            if (jhi - jlo + 1 >= w.nb || jlo < 0 || jhi >= w.nb) { jlo = 0; jhi = w.nb - 1; }
+        } else {
+            if (jhi < 0 || jlo > rg.m - 1) return;
+            if (jlo < 0) jlo = 0;
+            if (jhi > rg.m - 1) jhi = rg.m - 1;
+        }
+    }
+    const long long base = (long long)w.ring_rel * rg.m;
+    a = __ldg(bin_start + base + jlo);
+    n = __ldg(bin_start + base + jhi + 1) - a;
+}
+
+struct TaskConst {
+    uint32_t xc0, yc;
+    float c0, c1, c2, c3, du;
+    float qx, qy, h4max, k1, k2;
+};
+
+__device__ __forceinline__ TaskConst make_task_const(const ConvArgs& a, const Strip& st, int ix0) {
+    TaskConst tc;
+    const double u = st.u0 + (double)ix0 * st.du;
+    tc.xc0 = (uint32_t)(unsigned long long)__double2ll_rn(u * a.sx);
+    tc.yc = st.yi;
+    tc.c0 = st.c0; tc.c1 = st.c1; tc.c2 = st.c2; tc.c3 = st.c3; tc.du = st.du_f;
+    tc.qx = a.qx; tc.qy = a.qy; tc.h4max = a.kp.h4max; tc.k1 = a.kp.k1; tc.k2 = a.kp.k2;
+    return tc;
+}
+
+// Step (v), one cell: fp32 pair arithmetic on exact fixed-point differences (see
+// pair_update in convolve.cu for the derivation).  Returns d <= R and the kernel weight.
+__device__ __forceinline__ bool pair32(const Rec32& r, const TaskConst& tc, float& w) {
+    const float dx = (float)(int)(r.xi - tc.xc0) * tc.qx;
+    const float dy = (float)(int)(r.yi - tc.yc) * tc.qy;
+    const float u = dy * dy;
+    const float u2 = u * fmaf(u, -1.0f / 12.0f, 1.0f);
+    const float C = fmaf(dy, fmaf(dy, fmaf(dy, tc.c3, tc.c2), tc.c1), tc.c0);
+    const float v = dx * dx;
+    const float B = v * fmaf(v, -1.0f / 12.0f, 1.0f);
+    const float h4 = fmaf(C, B, u2);
+    w = ex2_approx(h4 * fmaf(h4, tc.k2, tc.k1));
+    return h4 <= tc.h4max;
+}
+
+// launcher of convolve_gen.cu
+int launch_conv_general(hcgrid_ctx* c, const ConvArgs& a, bool pair_f64, bool out_double, cudaStream_t st);
+
+}  // namespace hcg

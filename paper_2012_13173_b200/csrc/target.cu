@@ -1,0 +1,238 @@
+// target.cu -- step a1: target set-up.
+//
+// From the target cells and the kernel support radius R this derives (i) the REGION of
+// the sphere the target can reach -- the ring range [ring_first, ring_first + nring) and
+// the longitude window [lon_lo, lon_lo + wx) -- which fixes the layout of the ring table
+// and the per-pixel table, and (ii) per (strip, ring) the lookup-bin window of the
+// support disc, PAPER.md:136 step (i) "minimum and maximum ring indices within the range
+// of influence" and step (ii) "starting contributing pixel" of each ring.
+//
+// Disc geometry: a disc of radius R centred at latitude phi_c has, at latitude phi, the
+// longitude half-width dl with
+//     sin^2(dl/2) = [sin^2(R/2) - sin^2((phi - phi_c)/2)] / (cos(phi) cos(phi_c)),
+// maximal at sin(phi*) = sin(phi_c) / cos(R).  A point in HEALPix ring r has a latitude
+// between the centres of rings r+1 and r-1 (hcg_healpix.cuh fact 2), so the window of ring
+// r is the half-width at phi* clamped into that band (clipped to phi_c +- R).
+#include <algorithm>
+#include <cmath>
+#include <vector>
+
+#include "hcg_common.cuh"
+
+namespace hcg {
+
+__global__ void ring_window_kernel(const Strip* __restrict__ strips, RingWin* __restrict__ wins,
+                                   int nstrip, int kmax, Region rg, double radius) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (long long)nstrip * kmax) return;
+    const int s = (int)(t / kmax), k = (int)(t % kmax);
+    const Strip st = strips[s];
+    RingWin w;
+    w.a_lo = w.a_hi = w.step = 0.0;
+    w.ring_rel = st.ring_lo + k;
+    w.flags = 0;
+    w.nb = 0;
+    w.pad_ = 0;
+    if (k < st.nring) {
+        const int r = rg.ring_first + w.ring_rel;                  // HEALPix ring number
+        const double eps = 1e-10;
+        double band_hi = kHalfPi - ring_colat(r - 1, rg.nside) + eps;   // latitude band of ring r
+        double band_lo = kHalfPi - ring_colat(r + 1, rg.nside) - eps;
+        const double lo = fmax(band_lo, st.lat - radius);
+        const double hi = fmin(band_hi, st.lat + radius);
+        w.nb = (int)ring_nbins(r, rg.nside, rg.subpix);
+        if (lo <= hi) {
+            bool whole = fabs(st.lat) + radius >= kHalfPi - 1e-9;    // disc holds a pole
+            double dl = 0.0;
+            if (!whole) {
+                const double sstar = sin(st.lat) / cos(radius);
+                const double pstar = asin(fmin(1.0, fmax(-1.0, sstar)));
+                const double pe = fmin(hi, fmax(lo, pstar));
+                const double sr = sin(0.5 * radius), sd = sin(0.5 * (pe - st.lat));
+                const double f = (sr * sr - sd * sd) / (cos(pe) * cos(st.lat));
+                if (f >= 1.0) whole = true;
+                else dl = 2.0 * asin(sqrt(fmax(f, 0.0))) + 1e-9;
+            }
+            if (whole) {
+                w.flags = 2;
+            } else {
+                const double c = ldexp((double)ring_npix(r, rg.nside) / kTwoPi, rg.subpix);
+                const double g0 = ring_bin_coord(r, rg.nside, rg.lon_lo, rg.subpix);
+                const double frac0 = g0 - (floor(g0) - 2.0);       // in [2, 3)
+                w.a_lo = frac0 + (st.u0 - dl) * c;
+                w.a_hi = frac0 + (st.u0 + dl) * c;
+                w.step = st.du * c;
+                w.flags = 1;
+            }
+        }
+    }
+    wins[t] = w;
+}
+
+static double wrap_pm_pi(double x) {
+    x = fmod(x + kPi, kTwoPi);
+    if (x < 0) x += kTwoPi;
+    return x - kPi;
+}
+
+struct HostStrip { double lon0_deg, dlon_deg, lat_deg; };
+
+// Common tail of both set_target flavours: region, strips, ring windows.
+static int finish_target(hcgrid_ctx* c, const std::vector<HostStrip>& hs, int strip_cells,
+                         double west, double east /* unwrapped rad, of all cell centres */) {
+    const double R = c->kp.radius;
+    const int nside = c->nside;
+    double latmin = 1e9, latmax = -1e9, maxabs = 0;
+    for (const auto& h : hs) {
+        const double la = h.lat_deg * kDeg2Rad;
+        latmin = std::min(latmin, la); latmax = std::max(latmax, la);
+        maxabs = std::max(maxabs, std::fabs(la));
+    }
+    Region rg{};
+    rg.nside = nside;
+    // rings the target can reach (PAPER.md:136 step i over the whole target)
+    const double th_a = std::max(0.0, kHalfPi - (latmax + R));
+    const double th_b = std::min(kPi, kHalfPi - (latmin - R));
+    int rf = (int)std::floor(ring_coord(th_a, nside)) - 1;
+    int rl = (int)std::ceil(ring_coord(th_b, nside)) + 1;
+    rf = std::max(rf, 1); rl = std::min(rl, 4 * nside - 1);
+    rg.ring_first = rf;
+    rg.nring = rl - rf + 1;
+    const bool pole = maxabs + R >= kHalfPi - 1e-6;
+    const double dlmax = pole ? kPi : std::asin(std::min(1.0, std::sin(R) / std::cos(maxabs))) + 1e-9;
+    int npr_max = 0, npr_min = 1 << 30;
+    for (int r = rf; r <= rl; ++r) {
+        npr_max = std::max(npr_max, ring_npix(r, nside));
+        npr_min = std::min(npr_min, ring_npix(r, nside));
+    }
+    // sub-pixel bits: auto = 2 (quarter-pixel bins), reduced until the table fits
+    int b = c->opt_subpix > -100 ? c->opt_subpix : 2;
+    b = std::min(b, 6);
+    const int64_t cap = (int64_t)1 << 28;
+    for (;; --b) {
+        const double binw = kTwoPi / std::ldexp((double)npr_min, b);   // widest bin, rad
+        const double width = (east - west) + 2.0 * dlmax + 4.0 * binw + 1e-6;
+        const bool full = pole || width >= 0.98 * kTwoPi;
+        int64_t m;
+        if (full) {
+            m = 0;
+            for (int r = rf; r <= rl; ++r) m = std::max<int64_t>(m, ring_nbins(r, nside, b));
+        } else {
+            m = (int64_t)std::ceil(width * std::ldexp((double)npr_max / kTwoPi, b)) + 6;
+        }
+        if (m * rg.nring <= cap || b < -20) {
+            rg.subpix = b;
+            rg.m = (int32_t)m;
+            rg.full_circle = full ? 1 : 0;
+            if (full) { rg.lon_lo = 0.0; rg.wx = kTwoPi; }
+            else {
+                double lo = std::fmod(west - dlmax - 2.0 * binw - 5e-7, kTwoPi);
+                if (lo < 0) lo += kTwoPi;
+                rg.lon_lo = lo; rg.wx = width;
+            }
+            break;
+        }
+    }
+    if ((int64_t)rg.m * rg.nring > cap)
+        return fail(c, HCGRID_ERR_UNSUPPORTED, "lookup table too large (%lld bins)",
+                    (long long)rg.m * rg.nring);
+    rg.nbins = (int64_t)rg.m * rg.nring;
+    rg.lat_lo = kHalfPi - ring_colat(rl + 1, nside) - 1e-7;
+    const double lat_hi = kHalfPi - ring_colat(rf - 1, nside) + 1e-7;
+    rg.wy = lat_hi - rg.lat_lo;
+    c->region = rg;
+
+    // strips
+    std::vector<Strip> st(hs.size());
+    int kmax = 1;
+    double cw = 1e9;
+    const double sx = 4294967296.0 / rg.wx, sy = 4294967296.0 / rg.wy;
+    (void)sx;
+    for (size_t i = 0; i < hs.size(); ++i) {
+        Strip& s = st[i];
+        const HostStrip& h = hs[i];
+        s.lon0_deg = h.lon0_deg; s.dlon_deg = h.dlon_deg; s.lat_deg = h.lat_deg;
+        s.lat = h.lat_deg * kDeg2Rad;
+        double u = std::fmod(h.lon0_deg * kDeg2Rad - rg.lon_lo, kTwoPi);
+        if (u < 0) u += kTwoPi;
+        s.u0 = u;
+        s.du = h.dlon_deg * kDeg2Rad;
+        const double ta = std::max(0.0, kHalfPi - (s.lat + R));
+        const double tb = std::min(kPi, kHalfPi - (s.lat - R));
+        int a = std::max(rf, (int)std::floor(ring_coord(ta, nside)) - 1);
+        int bb = std::min(rl, (int)std::ceil(ring_coord(tb, nside)) + 1);
+        s.ring_lo = a - rf;
+        s.nring = bb - a + 1;
+        kmax = std::max(kmax, s.nring);
+        s.yi = (uint32_t)(long long)std::llrint((s.lat - rg.lat_lo) * sy);
+        const double cc = std::cos(s.lat), sc = std::sin(s.lat);
+        s.c0 = (float)(cc * cc); s.c1 = (float)(-cc * sc);
+        s.c2 = (float)(-0.5 * cc * cc); s.c3 = (float)(cc * sc / 6.0);
+        s.du_f = (float)s.du;
+        s.pad_ = 0;
+        if (strip_cells > 1) cw = std::min(cw, std::fabs(s.du) * cc);
+    }
+    c->kmax = kmax;
+    c->nstrip = (int32_t)hs.size();
+    c->strip_cells = strip_cells;
+    c->cell_width_sky = strip_cells > 1 ? cw : 0.0;
+    // small-angle series of the fp32 pair arithmetic: valid while R and the widest
+    // longitude half-window stay below 0.05 rad (dropped x^6/360 term < 2e-8 relative)
+    c->f32_series_ok = !pole && R <= 0.05 && dlmax <= 0.05;
+
+    HCG_CUDA(c, c->d_strips.ensure(st.size() * sizeof(Strip)));
+    HCG_CUDA(c, cudaMemcpy(c->d_strips.p, st.data(), st.size() * sizeof(Strip), cudaMemcpyHostToDevice));
+    const size_t nw = st.size() * (size_t)kmax;
+    HCG_CUDA(c, c->d_wins.ensure(nw * sizeof(RingWin)));
+    const int threads = 128;
+    const unsigned blocks = (unsigned)((nw + threads - 1) / threads);
+    ring_window_kernel<<<blocks, threads>>>(c->d_strips.as<Strip>(), c->d_wins.as<RingWin>(),
+                                            (int)st.size(), kmax, rg, R);
+    HCG_CUDA(c, cudaGetLastError());
+    HCG_CUDA(c, cudaDeviceSynchronize());
+    c->has_target = true;
+    return HCGRID_OK;
+}
+
+int build_target_car(hcgrid_ctx* c, int nx, int ny, double lon0, double lat0, double dlon, double dlat) {
+    std::vector<HostStrip> hs((size_t)ny);
+    for (int iy = 0; iy < ny; ++iy) {
+        volatile double prod = (double)iy * dlat;     // one rounding per operation, no FMA
+        volatile double la = lat0 + prod;
+        if (la > 90.0 || la < -90.0)
+            return fail(c, HCGRID_ERR_INVALID_ARG, "target row %d has latitude %.17g outside [-90, 90]", iy, (double)la);
+        hs[(size_t)iy] = HostStrip{lon0, dlon, la};
+    }
+    volatile double span = (double)(nx - 1) * dlon;
+    const double a = lon0 * kDeg2Rad, b = (lon0 + span) * kDeg2Rad;
+    c->is_car = true;
+    c->ncell = (int64_t)nx * ny;
+    return finish_target(c, hs, nx, std::min(a, b), std::max(a, b));
+}
+
+int build_target_cells(hcgrid_ctx* c, int64_t ncell, const double* lon, const double* lat, cudaStream_t st) {
+    std::vector<double> hl((size_t)ncell), hb((size_t)ncell);
+    HCG_CUDA(c, cudaMemcpyAsync(hl.data(), lon, sizeof(double) * (size_t)ncell, cudaMemcpyDeviceToHost, st));
+    HCG_CUDA(c, cudaMemcpyAsync(hb.data(), lat, sizeof(double) * (size_t)ncell, cudaMemcpyDeviceToHost, st));
+    HCG_CUDA(c, cudaStreamSynchronize(st));
+    std::vector<HostStrip> hs((size_t)ncell);
+    double sx = 0, sy = 0;
+    for (int64_t i = 0; i < ncell; ++i) {
+        if (!(hb[(size_t)i] >= -90.0 && hb[(size_t)i] <= 90.0) || !std::isfinite(hl[(size_t)i]))
+            return fail(c, HCGRID_ERR_INVALID_ARG, "target cell %lld has invalid coordinates", (long long)i);
+        hs[(size_t)i] = HostStrip{hl[(size_t)i], 0.0, hb[(size_t)i]};
+        sx += std::cos(hl[(size_t)i] * kDeg2Rad); sy += std::sin(hl[(size_t)i] * kDeg2Rad);
+    }
+    // longitude extent about the circular mean of the cells
+    const double lm = std::atan2(sy, sx);
+    double dmin = 0, dmax = 0;
+    for (int64_t i = 0; i < ncell; ++i) {
+        const double d = wrap_pm_pi(hl[(size_t)i] * kDeg2Rad - lm);
+        dmin = std::min(dmin, d); dmax = std::max(dmax, d);
+    }
+    c->is_car = false;
+    c->ncell = ncell;
+    return finish_target(c, hs, 1, lm + dmin, lm + dmax);
+}
+
+}  // namespace hcg

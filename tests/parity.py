@@ -1,0 +1,57 @@
+"""Comparison of a CUDA-path result with the oracle's, at the bar BASELINE.json's north_star
+states: counts bit-exact up to the pairs within 1e-9 rad of the
+support boundary, weight map and datacube within `tol` relative, NaN where W == 0."""
+import math
+
+import numpy as np
+
+TOL_F32 = 1e-5     # north_star: "within 1e-5 relative (fp32 accumulation)"
+TOL_F64 = 1e-12    # north_star: "or 1e-12 (fp64 mode)"
+
+
+def compare(cube, wmap, counts, ref, sigma_deg, radius_deg, tol, qmax=1.0, cells=None):
+    """ref: oracle.OracleResult (optionally of the subset `cells` of the flat cell index).
+    Returns a dict of the worst normalised errors; raises AssertionError on a violation."""
+    cube = np.asarray(cube, dtype=np.float64)
+    wmap = np.asarray(wmap, dtype=np.float64)
+    if cube.ndim == 1:
+        cube = cube[:, None]
+    if cells is not None:
+        cube, wmap = cube[cells], wmap[cells]
+        counts = None if counts is None else np.asarray(counts)[cells]
+    nb = ref.near_boundary
+    # a pair within 1e-9 rad of the boundary may fall on either side: it moves the count by
+    # one and W by at most q * exp(-R^2 / 2 sigma^2)
+    w_edge = qmax * math.exp(-0.5 * (radius_deg / sigma_deg) ** 2) * 1.001
+    if counts is not None:
+        dc = np.abs(np.asarray(counts, dtype=np.int64) - ref.counts)
+        bad = np.flatnonzero(dc > nb)
+        assert bad.size == 0, (f"{bad.size} cells with wrong contributing-sample count; first: cell {bad[0]} "
+                               f"gpu {int(np.asarray(counts)[bad[0]])} oracle {int(ref.counts[bad[0]])} "
+                               f"near-boundary {int(nb[bad[0]])}")
+    empty = ref.weightmap == 0
+    # weight map
+    errw = np.abs(wmap - ref.weightmap)
+    alloww = tol * ref.weightmap + nb * w_edge
+    badw = np.flatnonzero(errw > alloww)
+    assert badw.size == 0, (f"{badw.size} weight-map cells out of tolerance; first: cell {badw[0]} gpu "
+                            f"{wmap[badw[0]]!r} oracle {ref.weightmap[badw[0]]!r}")
+    # datacube
+    assert np.array_equal(np.isnan(cube), np.isnan(ref.datacube)), "NaN pattern (empty cells) differs"
+    ok = ~empty
+    scale = np.maximum(np.abs(ref.datacube[ok]), ref.absmap[ok])
+    errv = np.abs(cube[ok] - ref.datacube[ok])
+    # a boundary pair changes V by at most w_edge * (|v| + |V|) / W <= 2 w_edge * max|v| / W; bound it
+    # loosely through the cell's own scale (only cells with nb > 0 get the slack)
+    slack = (nb[ok] * w_edge / np.maximum(ref.weightmap[ok], 1e-300))[:, None] * 50.0 * np.maximum(scale, 1.0)
+    allowv = tol * scale + slack
+    badv = np.argwhere(errv > allowv)
+    assert badv.shape[0] == 0, (f"{badv.shape[0]} datacube entries out of tolerance; first: {badv[0]} gpu "
+                                f"{cube[ok][tuple(badv[0])]!r} oracle {ref.datacube[ok][tuple(badv[0])]!r}")
+    nz = ref.weightmap > 0
+    return {
+        "max_rel_w": float(np.max(errw[nz] / ref.weightmap[nz])) if nz.any() else 0.0,
+        "max_rel_v": float(np.max(errv / np.maximum(scale, 1e-300))) if ok.any() else 0.0,
+        "near_boundary_pairs": int(nb.sum()),
+        "n_hit": int(ref.counts.sum()),
+    }
