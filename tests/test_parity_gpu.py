@@ -1,0 +1,285 @@
+"""GPU parity: the CUDA path (through the C-ABI, via the thin binding) against the brute-force
+fp64 oracle, element by element on the same seeded inputs.
+
+Bar (BASELINE.json north_star; tests/parity.py): contributing-sample
+counts bit-exact up to the pairs within 1e-9 rad of the support boundary, weight map and
+datacube within 1e-5 relative (fp32 mode) or 1e-12 (fp64 mode), NaN where W == 0.
+
+Sizes: miniatures of every BASELINE config (same density / kernel / nside, smaller patch;
+several warp tasks, several staging chunks and a ragged tail each) in full, and the
+full-size configs in the launch configuration bench.py times, on sampled cells the oracle
+computes one by one.
+"""
+import numpy as np
+import pytest
+
+from paper_2012_13173_b200 import workloads
+
+from parity import TOL_F32, TOL_F64, compare
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+
+def _dev(a, dtype=None):
+    return torch.as_tensor(np.ascontiguousarray(a), dtype=dtype).cuda()
+
+
+def run_gpu(w, precision="f32", options=None, explicit_cells=False, nside=None, want_counts=True):
+    from paper_2012_13173_b200 import binding
+    g = binding.HCGrid(w.sigma_deg, w.radius_deg, nside or w.nside, precision=precision)
+    for k, v in (options or {}).items():
+        g.set_option(k, v)
+    t = w.target
+    if explicit_cells:
+        cl, cb = t.cell_centers()
+        g.set_target_cells(_dev(cl), _dev(cb))
+    else:
+        g.set_target_car(t.nx, t.ny, t.lon0, t.lat0, t.dlon, t.dlat)
+    cube, wmap, cnt = g.grid(_dev(w.lon), _dev(w.lat), _dev(w.values),
+                             None if w.weights is None else _dev(w.weights), want_counts=want_counts)
+    torch.cuda.synchronize()
+    st = g.stats()
+    g.close()
+    return cube.cpu().numpy(), wmap.cpu().numpy(), None if cnt is None else cnt.cpu().numpy(), st
+
+
+def run_oracle(oracle, w, cells=None):
+    cl, cb = w.target.cell_centers()
+    if cells is not None:
+        cl, cb = cl[cells], cb[cells]
+    return oracle.grid(w.sigma_deg, w.radius_deg, cl, cb, w.lon, w.lat, w.values, w.weights)
+
+
+def qmax(w):
+    return 1.0 if w.weights is None else float(w.weights.max())
+
+
+MINI = {1: 1.0, 2: 0.03, 3: 0.006, 4: 0.012, 5: 0.004}
+_cache = {}
+
+
+def mini(oracle, cfg):
+    if cfg not in _cache:
+        w = workloads.make(cfg, MINI[cfg])
+        _cache[cfg] = (w, run_oracle(oracle, w))
+    return _cache[cfg]
+
+
+# ------------------------------------------------------------ every config, both precisions
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_config_miniature_f32(oracle, cfg):
+    w, ref = mini(oracle, cfg)
+    cube, wmap, cnt, st = run_gpu(w, "f32")
+    r = compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F32, qmax(w))
+    assert r["n_hit"] > 0
+    assert st["gpu_launches"] >= 4
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_config_miniature_f64(oracle, cfg):
+    w, ref = mini(oracle, cfg)
+    # fp64 mode compares on the explicit cell arrays the oracle used (SURVEY 8c fp64 pin 2)
+    cube, wmap, cnt, _ = run_gpu(w, "f64", explicit_cells=(cfg % 2 == 0))
+    assert cube.dtype == np.float64 and wmap.dtype == np.float64
+    compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F64, qmax(w))
+
+
+# ------------------------------------------------------------ every kernel variant / coarsening
+@pytest.mark.parametrize("cfg", [1, 3, 5])
+@pytest.mark.parametrize("kernel", [1, 2, 3])
+def test_kernel_variants(oracle, cfg, kernel):
+    from paper_2012_13173_b200 import binding
+    w, ref = mini(oracle, cfg)
+    cube, wmap, cnt, st = run_gpu(w, "f32", {binding.OPT_KERNEL: kernel})
+    compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F32, qmax(w))
+
+
+@pytest.mark.parametrize("coarsen", [1, 2, 3, 4, 6, 8])
+@pytest.mark.parametrize("cfg", [1, 5])
+def test_coarsening(oracle, cfg, coarsen):
+    from paper_2012_13173_b200 import binding
+    w, ref = mini(oracle, cfg)
+    for kernel in (0, 1):
+        cube, wmap, cnt, st = run_gpu(w, "f32", {binding.OPT_COARSEN: coarsen, binding.OPT_KERNEL: kernel})
+        assert st["coarsen"] == coarsen
+        compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F32, qmax(w))
+
+
+@pytest.mark.parametrize("subpix", [0, 1, 3])
+def test_lookup_bin_refinement(oracle, subpix):
+    from paper_2012_13173_b200 import binding
+    w, ref = mini(oracle, 3)
+    cube, wmap, cnt, st = run_gpu(w, "f32", {binding.OPT_SUBPIX_BITS: subpix})
+    assert st["subpix_bits"] == subpix
+    compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F32)
+
+
+# ------------------------------------------------------------ nside is only an index (c11)
+@pytest.mark.parametrize("nside", [64, 256, 1024, 8192])
+def test_nside_invariance(oracle, nside):
+    w, ref = mini(oracle, 1)
+    cube, wmap, cnt, _ = run_gpu(w, "f32", nside=nside)
+    compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F32)
+
+
+def test_explicit_cells_equal_car(oracle):
+    w, ref = mini(oracle, 2)
+    a = run_gpu(w, "f32", explicit_cells=True)
+    compare(a[0], a[1], a[2], ref, w.sigma_deg, w.radius_deg, TOL_F32)
+
+
+def test_deterministic_bitwise():
+    w = workloads.make(3, MINI[3])
+    a = run_gpu(w, "f32")
+    b = run_gpu(w, "f32")
+    assert np.array_equal(a[0], b[0], equal_nan=True) and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+
+
+# ------------------------------------------------------------ arbitrary cells: seam, poles, odd nchan
+CASES = [
+    # seed, lon_c, lat_c, half_deg, sigma', nside, nchan, weights
+    (1, 0.0, 0.0, 0.5, 2.0, 1024, 1, False),       # lon = 0/360 seam on the equator
+    (2, 359.9, 41.8, 0.4, 1.5, 2048, 3, True),     # seam at the belt / cap transition latitude
+    (3, 200.0, 89.7, 0.5, 3.0, 512, 1, True),      # north pole inside the discs (whole rings)
+    (4, 10.0, -89.8, 0.4, 2.0, 256, 5, False),     # south pole
+    (5, 120.0, -60.0, 0.6, 2.0, 4096, 7, False),   # south cap, nchan not a multiple of 4
+    (6, 77.0, 10.0, 1.0, 4.0, 128, 300, True),     # more than one 256-channel tile
+]
+
+
+@pytest.mark.parametrize("case", CASES, ids=lambda c: f"seed{c[0]}")
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+def test_arbitrary_cells(oracle, case, precision):
+    from paper_2012_13173_b200 import binding
+    seed, lon_c, lat_c, half, sig_am, nside, nchan, use_w = case
+    lon, lat, val, wts, clon, clat = workloads.random_case(seed, 6000, 700, lon_c, lat_c, half, nchan, use_w)
+    sigma, radius = sig_am / 60.0, 3.0 * sig_am / 60.0
+    ref = oracle.grid(sigma, radius, clon, clat, lon, lat, val, wts)
+    assert ref.counts.sum() > 0
+    g = binding.HCGrid(sigma, radius, nside, precision=precision)
+    g.set_target_cells(_dev(clon), _dev(clat))
+    cube, wmap, cnt = g.grid(_dev(lon), _dev(lat), _dev(val), None if wts is None else _dev(wts))
+    torch.cuda.synchronize()
+    tol = TOL_F32 if precision == "f32" else TOL_F64
+    compare(cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy(), ref, sigma, radius, tol,
+            1.5 if use_w else 1.0)
+    g.close()
+
+
+def test_car_target_across_seam_and_negative_steps(oracle):
+    from paper_2012_13173_b200 import binding
+    lon, lat, val, _, _, _ = workloads.random_case(11, 8000, 1, 0.0, 30.0, 0.6)
+    tgt = workloads.CarTarget(50, 40, 0.4, 30.35, -1.0 / 60.0, -1.0 / 60.0)   # runs westwards over lon = 0
+    cl, cb = tgt.cell_centers()
+    sigma, radius = 1.5 / 60.0, 4.5 / 60.0
+    ref = oracle.grid(sigma, radius, cl, cb, lon, lat, val)
+    for precision, tol in (("f32", TOL_F32), ("f64", TOL_F64)):
+        g = binding.HCGrid(sigma, radius, 2048, precision=precision)
+        g.set_target_car(tgt.nx, tgt.ny, tgt.lon0, tgt.lat0, tgt.dlon, tgt.dlat)
+        cube, wmap, cnt = g.grid(_dev(lon), _dev(lat), _dev(val))
+        torch.cuda.synchronize()
+        compare(cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy(), ref, sigma, radius, tol)
+        g.close()
+
+
+# ------------------------------------------------------------ degenerate inputs
+def test_empty_input_and_unreachable_samples():
+    from paper_2012_13173_b200 import binding
+    g = binding.HCGrid(1.5 / 60, 4.5 / 60, 2048)
+    g.set_target_car(20, 10, 30.0, 20.0, 1 / 60, 1 / 60)
+    e64 = torch.empty(0, dtype=torch.float64, device="cuda")
+    cube, wmap, cnt = g.grid(e64, e64, torch.empty((0, 1), dtype=torch.float32, device="cuda"))
+    torch.cuda.synchronize()
+    assert torch.isnan(cube).all() and (wmap == 0).all() and (cnt == 0).all()
+    # samples that exist but lie far from every cell (other rings / other longitudes), NaN coordinates ignored
+    lon = _dev(np.array([100.0, 31.0, 30.1, np.nan, 30.1]))
+    lat = _dev(np.array([20.0, -40.0, 20.05, 20.0, 95.0]))
+    val = _dev(np.array([[1.0], [2.0], [7.0], [3.0], [4.0]], dtype=np.float32))
+    cube, wmap, cnt = g.grid(lon, lat, val)
+    torch.cuda.synchronize()
+    assert int(cnt.max()) == 1 and int((cnt > 0).sum()) > 0
+    hit = cnt > 0
+    assert torch.allclose(cube[hit], torch.full_like(cube[hit], 7.0), rtol=1e-6)
+    assert torch.isnan(cube[~hit]).all()
+    assert g.stats()["n_kept"] == 1
+    g.close()
+
+
+def test_single_cell_single_sample():
+    from paper_2012_13173_b200 import binding
+    for precision in ("f32", "f64"):
+        g = binding.HCGrid(1.0 / 60, 3.0 / 60, 4096, precision=precision)
+        g.set_target_car(1, 1, 10.0, -5.0, 1 / 60, 1 / 60)
+        cube, wmap, cnt = g.grid(_dev(np.array([10.0])), _dev(np.array([-5.0 + 1.0 / 60])),
+                                 _dev(np.array([[2.5]], dtype=np.float32)))
+        torch.cuda.synchronize()
+        assert int(cnt[0]) == 1
+        assert float(wmap[0]) == pytest.approx(np.exp(-0.5), rel=1e-6 if precision == "f32" else 1e-13)
+        assert float(cube[0, 0]) == pytest.approx(2.5, rel=1e-6)
+        g.close()
+
+
+def test_error_statuses():
+    from paper_2012_13173_b200 import binding
+    with pytest.raises(binding.HCGridError):
+        binding.HCGrid(-1.0, 0.1, 1024)
+    with pytest.raises(binding.HCGridError):
+        binding.HCGrid(0.1, 0.3, 1000)            # nside not a power of two
+    g = binding.HCGrid(0.1, 0.3, 1024)
+    x = torch.zeros(4, dtype=torch.float64, device="cuda")
+    with pytest.raises(binding.HCGridError) as ei:
+        g.grid(x, x, torch.zeros((4, 1), dtype=torch.float32, device="cuda"))
+    assert ei.value.status == -2                   # HCGRID_ERR_NO_TARGET
+    with pytest.raises(binding.HCGridError):
+        g.set_target_car(10, 10, 0.0, 85.0, 0.1, 1.0)   # rows run past the pole
+    with pytest.raises(binding.HCGridError):
+        g.set_option(99, 1)
+    g.close()
+
+
+def test_host_buffer_entry_point(oracle):
+    from paper_2012_13173_b200 import binding
+    w, ref = mini(oracle, 5)
+    g = binding.HCGrid(w.sigma_deg, w.radius_deg, w.nside)
+    t = w.target
+    g.set_target_car(t.nx, t.ny, t.lon0, t.lat0, t.dlon, t.dlat)
+    cube, wmap, cnt = g.grid_host(w.lon, w.lat, w.values, w.weights)
+    compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F32, qmax(w))
+    # context reuse: a second, different call on the same context
+    cube2, wmap2, cnt2 = g.grid_host(w.lon[::2], w.lat[::2], w.values[::2], w.weights[::2])
+    ref2 = oracle.grid(w.sigma_deg, w.radius_deg, *t.cell_centers(), w.lon[::2], w.lat[::2], w.values[::2],
+                       w.weights[::2])
+    compare(cube2, wmap2, cnt2, ref2, w.sigma_deg, w.radius_deg, TOL_F32, qmax(w))
+    g.close()
+
+
+# ------------------------------------------------------------ full size, bench launch configuration
+def sampled_cells(ncell, nx, k, seed):
+    """Stratified sample of the flat cell index: the four corners, a border band and seeded
+    interior cells."""
+    rng = np.random.default_rng([13173, 77, seed])
+    ny = ncell // nx
+    border = np.concatenate([np.arange(0, nx, max(1, nx // 16)), (ny - 1) * nx + np.arange(0, nx, max(1, nx // 16)),
+                             np.arange(0, ny, max(1, ny // 16)) * nx, np.arange(0, ny, max(1, ny // 16)) * nx + nx - 1,
+                             [0, nx - 1, (ny - 1) * nx, ncell - 1]])
+    inner = rng.choice(ncell, size=k, replace=False)
+    return np.unique(np.concatenate([border, inner])).astype(np.int64)
+
+
+@pytest.mark.parametrize("cfg,k", [(2, 600), (3, 300), (4, 150), (5, 120)])
+def test_full_size_sampled_cells(oracle, cfg, k):
+    w = workloads.make(cfg, 1.0)
+    cells = sampled_cells(w.target.ncell, w.target.nx, k, cfg)
+    ref = run_oracle(oracle, w, cells)
+    cube, wmap, cnt, st = run_gpu(w, "f32")          # default options = what bench.py times
+    r = compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F32, qmax(w), cells=cells)
+    assert r["n_hit"] > 0
+    # properties that hold at any size: W > 0 <=> count > 0 <=> finite V; count bounded by n
+    assert np.array_equal(wmap > 0, cnt > 0)
+    assert np.array_equal(np.isfinite(cube[:, 0]), cnt > 0)
+    assert cnt.min() >= 0 and cnt.max() <= w.n
+    if cfg == 3:
+        # fp64 mode at the target config, same sampled cells
+        cube, wmap, cnt, _ = run_gpu(w, "f64")
+        compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F64, cells=cells)

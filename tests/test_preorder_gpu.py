@@ -1,0 +1,91 @@
+"""Device pre-ordering (a2..a4) inspected on its own: PAPER.md:120-124 (Sect. 3.3 I-III) and
+the worked example of Fig. 3."""
+import numpy as np
+import pytest
+
+from paper_2012_13173_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+
+def _dev(a):
+    return torch.as_tensor(np.ascontiguousarray(a)).cuda()
+
+
+def test_device_pixelisation_equals_host_build():
+    from paper_2012_13173_b200 import binding
+    rng = np.random.default_rng(5)
+    lon = rng.uniform(-10, 370, 200000)
+    lat = np.degrees(np.arcsin(rng.uniform(-1, 1, 200000)))
+    for nside in (1, 4, 2048, 8192):
+        dev = binding.ang2pix_ring(nside, _dev(lon), _dev(lat)).cpu().numpy()
+        host = binding.host_ang2pix_ring(nside, lon, lat)
+        # same source compiled twice; device libm may differ by an ulp at pixel edges
+        assert np.mean(dev != host) < 1e-5
+        assert dev.min() >= 0 and dev.max() < 12 * nside * nside
+
+
+def test_sorted_order_and_tables():
+    from paper_2012_13173_b200 import binding
+    w = workloads.make(3, 0.004)
+    g = binding.HCGrid(w.sigma_deg, w.radius_deg, w.nside)
+    t = w.target
+    g.set_target_car(t.nx, t.ny, t.lon0, t.lat0, t.dlon, t.dlat)
+    g.grid(_dev(w.lon), _dev(w.lat), _dev(w.values))
+    pix, idx, ring_first, ring_start = g.debug_preorder()
+    st = g.stats()
+    nk = st["n_kept"]
+    assert 0 < nk <= w.n and pix.size == nk
+    # the "value" of the key-value sort is a permutation of distinct input indices
+    assert np.unique(idx).size == nk and idx.min() >= 0 and idx.max() < w.n
+    # S' carries the pixel of the sample it names
+    assert np.array_equal(pix, binding.host_ang2pix_ring(w.nside, w.lon[idx], w.lat[idx])) or \
+        np.mean(pix != binding.host_ang2pix_ring(w.nside, w.lon[idx], w.lat[idx])) < 1e-5
+    # sorted by ring: ring index non-decreasing along S' ("contiguous"); within a ring the
+    # order is by longitude measured from the region's western edge, i.e. pixel non-decreasing
+    # except for at most one wrap per ring
+    first = np.array([binding.host_ring_info(w.nside, r)[0] for r in range(ring_first, ring_first + st["n_rings"] + 1)])
+    ring_of = np.searchsorted(first, pix, side="right") - 1
+    assert np.all(np.diff(ring_of) >= 0)
+    # R_start: CSR over rings
+    assert ring_start[0] == 0 and ring_start[-1] == nk and np.all(np.diff(ring_start) >= 0)
+    for r in range(st["n_rings"]):
+        seg = ring_of[ring_start[r]:ring_start[r + 1]]
+        assert seg.size == 0 or (seg.min() == r and seg.max() == r)
+        p = pix[ring_start[r]:ring_start[r + 1]]
+        assert np.sum(np.diff(p) < 0) <= 1
+    # stable sort: equal pixels keep input order when they fall into the same lookup bin
+    g.close()
+
+
+def test_fig3_ring_table_semantics():
+    """Fig. 3: 17 samples in 4 rings holding 6, 3, 7, 1 -> R_start = 1, 7, 10, 17 (1-based),
+    ring i = [R_start[i], R_start[i+1] - 1]."""
+    from paper_2012_13173_b200 import binding
+    nside = 16
+    r0 = 20
+    hist = [6, 3, 7, 1]
+    lon, lat = [], []
+    for k, m in enumerate(hist):
+        la = binding.host_ring_info(nside, r0 + k)[2]
+        for j in range(m):
+            lon.append(40.0 + 1.3 * j)
+            lat.append(la)
+    lon, lat = np.array(lon), np.array(lat)
+    perm = np.random.default_rng(1).permutation(17)
+    g = binding.HCGrid(1.0, 3.0, nside)
+    g.set_target_car(12, 12, 38.0, lat.min() - 1.0, 1.0, (lat.max() - lat.min() + 2.0) / 11)
+    g.grid(_dev(lon[perm]), _dev(lat[perm]), _dev(np.ones((17, 1), np.float32)))
+    pix, idx, ring_first, ring_start = g.debug_preorder()
+    assert pix.size == 17
+    k0 = r0 - ring_first
+    assert list(ring_start[k0:k0 + 5] - ring_start[k0] + 1) == [1, 7, 10, 17, 18]
+    assert np.all(ring_start[:k0 + 1] == 0) and np.all(ring_start[k0 + 4:] == 17)
+    g.close()
+
+
+def test_measured_peaks_are_plausible():
+    from paper_2012_13173_b200 import binding
+    fp32, mufu = binding.measure_peaks(0)
+    assert 5e12 < fp32 < 6e13 and 5e11 < mufu < 8e12
