@@ -58,11 +58,15 @@ enum {
     HCGRID_OPT_PROFILE = 1,      /* 1: time every stage with CUDA events (hcgrid_get_stats) */
     HCGRID_OPT_SUBPIX_BITS = 2,  /* log2 of lookup bins per HEALPix pixel along the ring; -1 = auto.
                                     Takes effect at the next hcgrid_set_target_*. */
-    HCGRID_OPT_COARSEN = 3,      /* cells per warp task (thread coarsening); 0 = auto */
+    HCGRID_OPT_COARSEN = 3,      /* cells per warp task along a target row (thread coarsening,
+                                    PAPER.md:153, at warp scope); 0 = auto */
     HCGRID_OPT_KERNEL = 4,       /* 0 = auto; 1 = force the simple (non-staged) single-channel kernel;
                                     2 = force the fp64 pair arithmetic with the F32 output type;
-                                    3 = force the general (any nchan) kernel with fp32 pair arithmetic */
-    HCGRID_OPT_WARPS_PER_SM = 5  /* resident convolution warps per SM; 0 = auto */
+                                    3 = force the general (any nchan) kernel with fp32 pair arithmetic;
+                                    4 = force the TMA-staged single-channel kernel;
+                                    5 = force the tile kernel (error if the target does not allow it) */
+    HCGRID_OPT_WARPS_PER_SM = 5, /* resident convolution warps per SM (staged kernel); 0 = auto */
+    HCGRID_OPT_COARSEN_Y = 6     /* target rows per warp task (tile kernel); 0 = auto */
 };
 
 typedef struct {
@@ -71,10 +75,10 @@ typedef struct {
     int64_t n_bins;           /* entries of the per-pixel offset table                        */
     int32_t n_rings;          /* rings of the ring table                                      */
     int32_t subpix_bits;      /* lookup bins per HEALPix pixel = 2^subpix_bits (may be < 0)   */
-    int32_t coarsen;          /* cells per warp task used                                     */
+    int32_t coarsen;          /* cells per warp task along a row used                         */
     int32_t kernel;           /* convolution kernel variant that ran          */
     int32_t gpu_launches;     /* kernels launched by the last hcgrid_grid                     */
-    int32_t reserved;
+    int32_t coarsen_y;        /* target rows per warp task used (tile kernel; else 1)         */
     float us_pixelise, us_sort, us_tables, us_pack, us_convolve, us_total; /* PROFILE only   */
 } hcgrid_stats;
 

@@ -82,7 +82,7 @@ int hcgrid_create(hcgrid_ctx** out, double sigma_deg, double support_radius_deg,
 int hcgrid_destroy(hcgrid_ctx* c) {
     if (!c) return HCGRID_OK;
     cudaSetDevice(c->device);
-    DevBuf* bufs[] = {&c->d_strips, &c->d_wins, &c->d_cell_lon, &c->d_cell_lat, &c->d_keys, &c->d_keys_out,
+    DevBuf* bufs[] = {&c->d_strips, &c->d_wins, &c->d_winsf, &c->d_rowsf, &c->d_cell_lon, &c->d_cell_lat, &c->d_keys, &c->d_keys_out,
                       &c->d_idx, &c->d_idx_out, &c->d_sort_tmp, &c->d_bins, &c->d_rec, &c->d_misc,
                       &c->d_in_lon, &c->d_in_lat, &c->d_in_val, &c->d_in_wgt, &c->d_out_cube, &c->d_out_w,
                       &c->d_out_cnt};
@@ -105,8 +105,12 @@ int hcgrid_set_option(hcgrid_ctx* c, int option, int64_t value) {
             c->opt_coarsen = (int)value;
             break;
         case HCGRID_OPT_KERNEL:
-            if (value < 0 || value > 3) return fail(c, HCGRID_ERR_INVALID_ARG, "kernel must be 0..3");
+            if (value < 0 || value > 5) return fail(c, HCGRID_ERR_INVALID_ARG, "kernel must be 0..5");
             c->opt_kernel = (int)value;
+            break;
+        case HCGRID_OPT_COARSEN_Y:
+            if (value < 0 || value > 4) return fail(c, HCGRID_ERR_INVALID_ARG, "coarsen_y must be 0 (auto) or 1..4");
+            c->opt_coarsen_y = (int)value;
             break;
         case HCGRID_OPT_WARPS_PER_SM:
             if (value < 0 || value > 64) return fail(c, HCGRID_ERR_INVALID_ARG, "warps per SM must be 0..64");

@@ -283,7 +283,6 @@ static int launch_f32(hcgrid_ctx* c, ConvArgs& a, bool hasq, bool staged, cudaSt
 
 int run_convolve(hcgrid_ctx* c, int64_t n, const float* values, int nchan, bool has_weights, void* cube,
                  void* wmap, int32_t* counts, cudaStream_t st) {
-    (void)n;
     const Region& rg = c->region;
     ConvArgs a{};
     a.strips = c->d_strips.as<Strip>();
@@ -300,7 +299,14 @@ int run_convolve(hcgrid_ctx* c, int64_t n, const float* values, int nchan, bool 
     a.sx = 4294967296.0 / rg.wx;
     const bool f32 = c->precision == HCGRID_F32 && c->f32_series_ok && c->opt_kernel != 2;
     int rc;
-    if (f32 && nchan == 1 && c->opt_kernel != 3) {
+    c->stats.coarsen_y = 1;
+    if (c->opt_kernel == 5 && !(f32 && nchan == 1 && c->tile_ok))
+        return fail(c, HCGRID_ERR_UNSUPPORTED, "the tile kernel needs fp32 mode, one channel and a plate-carree "
+                    "target whose reach is a plain longitude window");
+    if (f32 && nchan == 1 && c->tile_ok && (c->opt_kernel == 0 || c->opt_kernel == 5)) {
+        rc = launch_conv_tile(c, n, (float*)cube, (float*)wmap, counts, st);
+        c->stats.kernel = 6;
+    } else if (f32 && nchan == 1 && c->opt_kernel != 3) {
         const bool staged = c->opt_kernel != 1 && c->kmax <= 32;
         int G = c->opt_coarsen;
         if (G == 0) G = c->strip_cells >= 4 ? 2 : 1;
@@ -308,11 +314,9 @@ int run_convolve(hcgrid_ctx* c, int64_t n, const float* values, int nchan, bool 
         switch (G) {
             case 1: rc = launch_f32<1>(c, a, has_weights, staged, st); break;
             case 2: rc = launch_f32<2>(c, a, has_weights, staged, st); break;
-            case 3: rc = launch_f32<3>(c, a, has_weights, staged, st); break;
             case 4: rc = launch_f32<4>(c, a, has_weights, staged, st); break;
-            case 6: rc = launch_f32<6>(c, a, has_weights, staged, st); break;
             case 8: rc = launch_f32<8>(c, a, has_weights, staged, st); break;
-            default: return fail(c, HCGRID_ERR_INVALID_ARG, "coarsen %d not built (1,2,3,4,6,8)", G);
+            default: return fail(c, HCGRID_ERR_INVALID_ARG, "coarsen %d not built (1,2,4,8)", G);
         }
         c->stats.coarsen = G;
         c->stats.kernel = staged ? 2 : 1;

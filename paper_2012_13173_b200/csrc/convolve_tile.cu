@@ -1,0 +1,354 @@
+// convolve_tile.cu -- step a6, the tile kernel: single-channel fp32 gather convolution for
+// plate-carree targets (Sect. 3.4 i-v; Eq. 1; kernel
+// PAPER.md:186), hand-written for sm_100a.  DESIGN.md "a6 / tile kernel".
+//
+// One WARP owns a tile of GX x GY target cells (the paper's thread coarsening,
+// PAPER.md:153, in two dimensions and at warp scope); its 32 lanes stride over the
+// candidate samples of the tile, so each lane holds one sample and GX*GY partial sums.
+//   step (i)    rings of the tile = union of its rows' precomputed ring ranges (a1)
+//   step (ii)   lane k turns ring k's window (fp32 RingWinF of every tile row, united) into
+//               a range of lookup bins
+//   step (iii)  two reads of the per-pixel table give the sample range [S_start, S_end)
+//   step (iv)   the ranges of all rings form one candidate stream: a 32-entry table
+//               (end position, address offset) per warp in shared memory lets every lane
+//               walk the stream with a monotone ring cursor; records are read straight
+//               from global memory (16-byte loads, one step ahead of the arithmetic)
+//   step (v)    pair arithmetic in fp32 on exact fixed-point coordinate differences, with
+//               everything that depends only on the sample's column or row offset hoisted
+//               out of the GX*GY pair loop and all lengths pre-scaled by
+//               sqrt(log2(e) / (2 sigma^2)), so a pair costs FFMA (distance), FSETP
+//               (d <= R), MUFU.EX2, FFMA (W), FFMA (sum) [+ IADD (count)].
+// The 32 partial sums per cell are combined by a transposed butterfly (each shuffle step
+// halves the number of live values), in a fixed order, without atomics.
+#include "hcg_conv.cuh"
+
+namespace hcg {
+
+struct TileArgs {
+    const RowF* rows;
+    const RingWinF* wins;
+    const int32_t* bin_start;
+    const Rec32* rec;
+    float* cube;
+    float* wmap;
+    int32_t* counts;
+    double u0, du, sx;          // lon offset of column 0 (rad), column step (rad), fixed-point units per rad
+    int32_t nx, ny, kmax, m;    // target shape, window-table row length, lookup bins per ring
+    int32_t tiles_x;
+    int64_t ntiles;
+    float sxk, syk;             // sqrt(kappa) * radians per fixed-point unit (lon, lat)
+    float duk, dyk;             // sqrt(kappa) * column step / row step (signed)
+    float isk;                  // 1 / sqrt(kappa)
+    float a12;                  // 1 / (12 kappa): series coefficient in scaled units
+    float hmax;                 // kappa * 4 sin^2(R/2)  (series modes)  or  kappa * R^2 (flat mode)
+};
+
+template <int GY>
+struct TileConst {
+    uint32_t xc0, yc0;
+    float sxk, syk, duk, dyk;
+    float cc0, p1, p2, p3;      // cos(lat_s) = cc0 + dy (p1 + dy (p2 + dy p3)), dy scaled
+    float cc[GY];
+    float a12, hmax;
+};
+
+// MODE 0 "flat": d^2 = dy^2 + cos cos dx^2 (valid while R^2/12 and dl_max^2/12 < 1e-7);
+// MODE 1 "series": 4 hav(d) = u(1-u/12) + C v(1-v/12) for the test, weight from the same;
+// MODE 2 "full": as 1, plus d^2 = h(1 + h/12) for the weight.
+template <int GX, int GY, int MODE, bool COUNTS>
+__device__ __forceinline__ void tile_pairs(const uint4 raw, const TileConst<GY>& tc, float (&W)[GX * GY],
+                                           float (&S)[GX * GY], int (&cnt)[GX * GY]) {
+    const float q = __uint_as_float(raw.w);
+    const float qv = q * __uint_as_float(raw.z);
+    const float dx0 = (float)(int)(raw.x - tc.xc0) * tc.sxk;
+    const float dy0 = (float)(int)(raw.y - tc.yc0) * tc.syk;
+    const float cs = fmaf(dy0, fmaf(dy0, fmaf(dy0, tc.p3, tc.p2), tc.p1), tc.cc0);
+    float V[GX], U[GY], C[GY];
+#pragma unroll
+    for (int i = 0; i < GX; ++i) {
+        const float dx = fmaf(-(float)i, tc.duk, dx0);
+        const float v = dx * dx;
+        V[i] = MODE >= 1 ? v * fmaf(v, -tc.a12, 1.0f) : v;
+    }
+#pragma unroll
+    for (int j = 0; j < GY; ++j) {
+        const float dy = fmaf(-(float)j, tc.dyk, dy0);
+        const float u = dy * dy;
+        U[j] = MODE >= 1 ? u * fmaf(u, -tc.a12, 1.0f) : u;
+        C[j] = tc.cc[j] * cs;
+    }
+#pragma unroll
+    for (int j = 0; j < GY; ++j) {
+#pragma unroll
+        for (int i = 0; i < GX; ++i) {
+            const float h = fmaf(C[j], V[i], U[j]);
+            const float e = MODE == 2 ? h * fmaf(h, tc.a12, 1.0f) : h;
+            const float w = ex2_approx(-e);
+            if (h <= tc.hmax) {
+                W[j * GX + i] = fmaf(w, q, W[j * GX + i]);
+                S[j * GX + i] = fmaf(w, qv, S[j * GX + i]);
+                if (COUNTS) cnt[j * GX + i] += 1;
+            }
+        }
+    }
+}
+
+// Transposed warp reduction of N (a power of two <= 32) per-lane values: after the call
+// v[0] of lane L holds the sum over all 32 lanes of value number L >> (5 - log2 N).
+template <int N, int SH, typename T>
+struct TileReduce {
+    static __device__ __forceinline__ void run(T* v, int lane) {
+        if constexpr (SH >= 1) {
+            if constexpr (N > 1) {
+                constexpr int H = N / 2;
+                const bool up = (lane & SH) != 0;
+#pragma unroll
+                for (int i = 0; i < H; ++i) {
+                    const T keep = up ? v[i + H] : v[i];
+                    const T send = up ? v[i] : v[i + H];
+                    v[i] = keep + __shfl_xor_sync(0xffffffffu, send, SH);
+                }
+                TileReduce<H, SH / 2, T>::run(v, lane);
+            } else {
+                v[0] += __shfl_xor_sync(0xffffffffu, v[0], SH);
+                TileReduce<1, SH / 2, T>::run(v, lane);
+            }
+        }
+    }
+};
+
+constexpr int ilog2(int n) { return n <= 1 ? 0 : 1 + ilog2(n / 2); }
+
+constexpr int kTileWarps = 4;
+
+template <int GX, int GY, int MODE, bool COUNTS>
+__global__ void __launch_bounds__(kTileWarps * 32)
+conv1_tile_f32(const TileArgs a) {
+    constexpr int NC = GX * GY;
+    __shared__ int2 s_tab[kTileWarps][32];
+    const int lane = threadIdx.x & 31;
+    const int wib = threadIdx.x >> 5;
+    const int64_t tile = (int64_t)blockIdx.x * kTileWarps + wib;
+    if (tile >= a.ntiles) return;
+    const int ty = (int)(tile / a.tiles_x);
+    const int ix0 = (int)(tile - (int64_t)ty * a.tiles_x) * GX;
+    const int row0 = ty * GY;
+    const int ncols = min(GX, a.nx - ix0);
+    const int nrows = min(GY, a.ny - row0);
+
+    // ---- tile constants
+    TileConst<GY> tc;
+    int ring_lo[GY], nring[GY];
+    int rmin = 0x7fffffff, rmax = -0x7fffffff;
+#pragma unroll
+    for (int j = 0; j < GY; ++j) {
+        const int4* rp = (const int4*)(a.rows + min(row0 + j, a.ny - 1));
+        const int4 r0 = __ldg(rp);
+        const int4 r1 = __ldg(rp + 1);
+        ring_lo[j] = r0.y;
+        nring[j] = j < nrows ? r0.z : 0;
+        tc.cc[j] = __int_as_float(r0.w);
+        if (j == 0) {
+            tc.yc0 = (uint32_t)r0.x;
+            tc.cc0 = __int_as_float(r0.w);
+            const float sc0 = __int_as_float(r1.x);
+            const float ik = a.isk;
+            tc.p1 = -sc0 * ik;
+            tc.p2 = -0.5f * tc.cc0 * ik * ik;
+            tc.p3 = sc0 * ik * ik * ik * (1.0f / 6.0f);
+        }
+        if (j < nrows) {
+            rmin = min(rmin, r0.y);
+            rmax = max(rmax, r0.y + r0.z - 1);
+        }
+    }
+    tc.xc0 = (uint32_t)(unsigned long long)__double2ll_rn((a.u0 + (double)ix0 * a.du) * a.sx);
+    tc.sxk = a.sxk; tc.syk = a.syk; tc.duk = a.duk; tc.dyk = a.dyk;
+    tc.a12 = a.a12; tc.hmax = a.hmax;
+
+    float W[NC], S[NC];
+    int cnt[NC];
+#pragma unroll
+    for (int c = 0; c < NC; ++c) { W[c] = 0.f; S[c] = 0.f; cnt[c] = 0; }
+
+    const float fxw = (float)(a.du >= 0.0 ? ix0 : ix0 + ncols - 1);   // westmost / eastmost column of the tile
+    const float fxe = (float)(a.du >= 0.0 ? ix0 + ncols - 1 : ix0);
+    const Rec32* __restrict__ rec = a.rec;
+    int2* tab = s_tab[wib];
+
+    for (int rb = rmin; rb <= rmax; rb += 32) {
+        // ---- steps (ii)+(iii): lane k <-> ring rb + k
+        const int r = rb + lane;
+        int jlo = 0x7fffffff, jhi = -1;
+#pragma unroll
+        for (int j = 0; j < GY; ++j) {
+            const int k = r - ring_lo[j];
+            if (k >= 0 && k < nring[j]) {
+                const float4 w = __ldg((const float4*)(a.wins + (size_t)(row0 + j) * a.kmax + k));
+                const int fl = __float_as_int(w.w);
+                if (fl == 1) {
+                    jlo = min(jlo, __float2int_rd(fmaf(fxw, w.z, w.x)));
+                    jhi = max(jhi, __float2int_rd(fmaf(fxe, w.z, w.y)));
+                } else if (fl == 2) {
+                    jlo = 0; jhi = a.m - 1;
+                }
+            }
+        }
+        jlo = max(jlo, 0);
+        jhi = min(jhi, a.m - 1);
+        int sa = 0, sn = 0;
+        if (jhi >= jlo) {
+            const int32_t* bs = a.bin_start + (size_t)r * a.m;
+            sa = __ldg(bs + jlo);
+            sn = __ldg(bs + jhi + 1) - sa;
+        }
+        int incl = sn;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += t;
+        }
+        const int total = __shfl_sync(0xffffffffu, incl, 31);
+        __syncwarp();                                   // previous pass done with the table
+        tab[lane] = make_int2(incl, sa - (incl - sn)); // (end of ring k in the stream, address offset)
+        __syncwarp();
+
+        // ---- steps (iv)+(v): the candidate stream, one record ahead
+        int i = lane;
+        if (i < total) {
+            int k = 0;
+            int2 t = tab[0];
+            while (i >= t.x) t = tab[++k];
+            uint4 nxt = __ldg((const uint4*)(rec + (t.y + i)));
+            while (true) {
+                const uint4 cur = nxt;
+                const int i2 = i + 32;
+                const bool more = i2 < total;
+                if (more) {
+                    while (i2 >= t.x) t = tab[++k];
+                    nxt = __ldg((const uint4*)(rec + (t.y + i2)));
+                }
+                tile_pairs<GX, GY, MODE, COUNTS>(cur, tc, W, S, cnt);
+                if (!more) break;
+                i = i2;
+            }
+        }
+    }
+
+    // ---- finish: transposed reduction, normalise, store
+    TileReduce<NC, 16, float>::run(W, lane);
+    TileReduce<NC, 16, float>::run(S, lane);
+    if (COUNTS) TileReduce<NC, 16, int>::run(cnt, lane);
+    constexpr int SHIFT = 5 - ilog2(NC);
+    if ((lane & ((1 << SHIFT) - 1)) == 0) {
+        const int c = lane >> SHIFT;
+        const int gx = c % GX, gy = c / GX;
+        if (gx < ncols && gy < nrows) {
+            const int64_t cell = (int64_t)(row0 + gy) * a.nx + ix0 + gx;
+            const float w = W[0];
+            a.cube[cell] = w > 0.0f ? S[0] / w : __int_as_float(0x7fc00000);
+            a.wmap[cell] = w;
+            if (COUNTS) a.counts[cell] = cnt[0];
+        }
+    }
+}
+
+// ------------------------------------------------------------------ launcher
+template <int GX, int GY>
+static cudaError_t launch_shape(const TileArgs& a, int mode, bool counts, cudaStream_t st) {
+    const unsigned blocks = (unsigned)((a.ntiles + kTileWarps - 1) / kTileWarps);
+    const int threads = kTileWarps * 32;
+#define HCG_TILE(M, C) conv1_tile_f32<GX, GY, M, C><<<blocks, threads, 0, st>>>(a)
+    switch (mode * 2 + (counts ? 1 : 0)) {
+        case 0: HCG_TILE(0, false); break;
+        case 1: HCG_TILE(0, true); break;
+        case 2: HCG_TILE(1, false); break;
+        case 3: HCG_TILE(1, true); break;
+        case 4: HCG_TILE(2, false); break;
+        default: HCG_TILE(2, true); break;
+    }
+#undef HCG_TILE
+    return cudaGetLastError();
+}
+
+static const int kShapes[][2] = {{1, 1}, {2, 1}, {4, 1}, {8, 1}, {2, 2}, {4, 2}, {8, 2}, {4, 4}};
+
+// Instruction-count model of one tile: warp instructions per cell.
+static double shape_cost(int gx, int gy, int mode, bool counts, double cw, double ch, double two_r,
+                         double ring_sp, double cand_per_cell) {
+    const double infl = (two_r + (gx - 1) * cw) / two_r * (two_r + 2.0 * ring_sp + (gy - 1) * ch) / (two_r + 2.0 * ring_sp);
+    const double per_iter = 18.0 + (mode >= 1 ? 4.0 : 2.0) * gx + (mode >= 1 ? 5.0 : 3.0) * gy +
+                            (5.0 + (counts ? 1.0 : 0.0) + (mode == 2 ? 2.0 : 0.0)) * gx * gy;
+    const double iters = cand_per_cell * infl / 32.0 + 0.5;
+    const double overhead = 150.0 + 14.0 * gy + 8.0 * gx * gy;
+    return (iters * per_iter + overhead) / (gx * gy);
+}
+
+int launch_conv_tile(hcgrid_ctx* c, int64_t n, float* cube, float* wmap, int32_t* counts, cudaStream_t st) {
+    const Region& rg = c->region;
+    const KernelParams& kp = c->kp;
+    const int nx = c->strip_cells, ny = c->nstrip;
+    const double kappa = 1.4426950408889634074 * kp.inv2s2;
+    const double sk = std::sqrt(kappa);
+    // which terms of the small-angle series the tolerances need
+    const double amax = std::max(c->dlmax, kp.radius);
+    const bool need_xy = amax * amax / 12.0 > 1e-7;
+    const bool need_d = kp.radius * kp.radius * kp.inv2s2 * (kp.radius * kp.radius / 12.0) > 1e-6;
+    const int mode = need_d ? 2 : (need_xy ? 1 : 0);
+
+    // tile shape: forced by the options or chosen by the instruction-count model
+    int gx = c->opt_coarsen, gy = c->opt_coarsen_y;
+    if (gx == 0 || gy == 0) {
+        const double two_r = 2.0 * kp.radius;
+        const double ring_sp = rg.wy / std::max(1, rg.nring);
+        // candidates of one cell's own search: samples per unit area x bounding box of the disc
+        const double dens = (double)n / std::max(1e-300, rg.wx * rg.wy);
+        const double cand = dens * (2.0 * c->dlmax) * (two_r + 2.0 * ring_sp);
+        double best = 1e300;
+        int bx = 1, by = 1;
+        for (const auto& s : kShapes) {
+            if ((gx != 0 && s[0] != gx) || (gy != 0 && s[1] != gy)) continue;
+            if (s[0] > nx && s[0] > 1) continue;
+            if (s[1] > ny && s[1] > 1) continue;
+            const double cost = shape_cost(s[0], s[1], mode, counts != nullptr, c->cell_width_sky,
+                                           std::fabs(c->car_dlat), two_r, ring_sp, cand);
+            if (cost < best) { best = cost; bx = s[0]; by = s[1]; }
+        }
+        if (best == 1e300)
+            return fail(c, HCGRID_ERR_INVALID_ARG, "tile shape %d x %d not built", gx, gy);
+        gx = bx; gy = by;
+    }
+
+    TileArgs a{};
+    a.rows = c->d_rowsf.as<RowF>();
+    a.wins = c->d_winsf.as<RingWinF>();
+    a.bin_start = c->d_bins.as<int32_t>();
+    a.rec = c->d_rec.as<Rec32>();
+    a.cube = cube; a.wmap = wmap; a.counts = counts;
+    a.u0 = c->car_u0; a.du = c->car_du; a.sx = 4294967296.0 / rg.wx;
+    a.nx = nx; a.ny = ny; a.kmax = c->kmax; a.m = rg.m;
+    a.tiles_x = (nx + gx - 1) / gx;
+    a.ntiles = (int64_t)a.tiles_x * ((ny + gy - 1) / gy);
+    a.sxk = (float)(sk * rg.wx / 4294967296.0);
+    a.syk = (float)(sk * rg.wy / 4294967296.0);
+    a.duk = (float)(sk * c->car_du);
+    a.dyk = (float)(sk * c->car_dlat);
+    a.isk = (float)(1.0 / sk);
+    a.a12 = (float)(1.0 / (12.0 * kappa));
+    a.hmax = (float)(mode == 0 ? kappa * kp.radius * kp.radius : kappa * 4.0 * kp.hav_max);
+
+    cudaError_t e = cudaSuccess;
+    bool built = false;
+#define HCG_SHAPE(X, Y) if (gx == X && gy == Y) { built = true; e = launch_shape<X, Y>(a, mode, counts != nullptr, st); }
+    HCG_SHAPE(1, 1); HCG_SHAPE(2, 1); HCG_SHAPE(4, 1); HCG_SHAPE(8, 1);
+    HCG_SHAPE(2, 2); HCG_SHAPE(4, 2); HCG_SHAPE(8, 2); HCG_SHAPE(4, 4);
+#undef HCG_SHAPE
+    if (!built)
+        return fail(c, HCGRID_ERR_INVALID_ARG, "tile shape %d x %d not built", gx, gy);
+    if (e != cudaSuccess) return cuda_fail(c, e, "conv1_tile_f32");
+    c->stats.coarsen = gx;
+    c->stats.coarsen_y = gy;
+    return HCGRID_OK;
+}
+
+}  // namespace hcg

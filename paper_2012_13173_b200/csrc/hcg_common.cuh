@@ -42,6 +42,26 @@ struct RingWin {
     int32_t pad_;
 };
 
+// fp32 form of RingWin for the tile kernel (convolve_tile.cu): the same window with the
+// bounds rounded outwards by the worst-case fp32 evaluation error, so that
+//   first bin = floor(a_lo + ix_west * step),  last bin = floor(a_hi + ix_east * step)
+// evaluated in fp32 is a superset of the fp64 window.  Entry k of a strip's row is ring
+// strip.ring_lo + k.  flags as in RingWin.
+struct __align__(16) RingWinF {
+    float a_lo, a_hi, step;
+    int32_t flags;
+};
+
+// Per-strip constants of the tile kernel (32 bytes, read with two 16-byte loads).
+struct __align__(16) RowF {
+    uint32_t yi;      // fixed-point latitude of the row (Rec32 convention)
+    int32_t ring_lo;  // first ring (relative to region ring_first) of the row's window table
+    int32_t nring;    // entries used in the row's window table
+    float cc;         // cos(lat_c)
+    float sc;         // sin(lat_c)
+    int32_t pad_[3];
+};
+
 // 16-byte packed sample S' as the fp32 convolution reads it (a5).  xi/yi are unsigned
 // fixed point over the region: lon offset u in [0, wx) -> xi = u / wx * 2^32 (wraps
 // naturally when wx = 2 pi), lat offset -> yi.  Differences of two fixed-point
@@ -108,7 +128,7 @@ struct hcgrid_ctx {
     int num_sms = 148;
     hcg::KernelParams kp{};
     // options
-    int opt_profile = 0, opt_subpix = -1000, opt_coarsen = 0, opt_kernel = 0, opt_warps = 0;
+    int opt_profile = 0, opt_subpix = -1000, opt_coarsen = 0, opt_coarsen_y = 0, opt_kernel = 0, opt_warps = 0;
     // target
     bool has_target = false;
     bool is_car = false;
@@ -117,7 +137,11 @@ struct hcgrid_ctx {
     bool f32_series_ok = true;      // small-angle series valid over the whole target
     double cell_width_sky = 0.0;    // min over strips of |du| cos(lat), rad (coarsening choice)
     hcg::Region region{};
-    hcg::DevBuf d_strips, d_wins, d_cell_lon, d_cell_lat;
+    hcg::DevBuf d_strips, d_wins, d_winsf, d_rowsf, d_cell_lon, d_cell_lat;
+    double car_u0 = 0.0, car_du = 0.0;   // plate-carree target: lon offset of column 0 / column step, rad
+    double car_dlat = 0.0;               // row step, rad (signed)
+    double dlmax = 0.0;                  // widest longitude half-window of a support disc, rad
+    bool tile_ok = false;                // the tile kernel's preconditions hold for this target
     // per-call scratch
     hcg::DevBuf d_keys, d_keys_out, d_idx, d_idx_out, d_sort_tmp, d_bins, d_rec, d_misc;
     hcg::DevBuf d_in_lon, d_in_lat, d_in_val, d_in_wgt, d_out_cube, d_out_w, d_out_cnt;  // *_host path

@@ -22,7 +22,8 @@
 namespace hcg {
 
 __global__ void ring_window_kernel(const Strip* __restrict__ strips, RingWin* __restrict__ wins,
-                                   int nstrip, int kmax, Region rg, double radius) {
+                                   RingWinF* __restrict__ winsf, int nstrip, int kmax, Region rg,
+                                   double radius) {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= (long long)nstrip * kmax) return;
     const int s = (int)(t / kmax), k = (int)(t % kmax);
@@ -67,6 +68,15 @@ __global__ void ring_window_kernel(const Strip* __restrict__ strips, RingWin* __
         }
     }
     wins[t] = w;
+    // fp32 copy, bounds moved outwards by the fp32 evaluation error of a + ix * step
+    // (|a + ix step| < m + 4, two roundings of 2^-24 relative each, plus step's own)
+    const double slack = 2.5e-7 * ((double)rg.m + 8.0) + 1e-4;
+    RingWinF f;
+    f.a_lo = __double2float_rd(w.a_lo - slack);
+    f.a_hi = __double2float_ru(w.a_hi + slack);
+    f.step = (float)w.step;
+    f.flags = w.flags;
+    winsf[t] = f;
 }
 
 static double wrap_pm_pi(double x) {
@@ -184,10 +194,25 @@ static int finish_target(hcgrid_ctx* c, const std::vector<HostStrip>& hs, int st
     HCG_CUDA(c, cudaMemcpy(c->d_strips.p, st.data(), st.size() * sizeof(Strip), cudaMemcpyHostToDevice));
     const size_t nw = st.size() * (size_t)kmax;
     HCG_CUDA(c, c->d_wins.ensure(nw * sizeof(RingWin)));
+    HCG_CUDA(c, c->d_winsf.ensure(nw * sizeof(RingWinF)));
+    std::vector<RowF> rows(st.size());
+    for (size_t i = 0; i < st.size(); ++i) {
+        RowF& r = rows[i];
+        r.yi = st[i].yi; r.ring_lo = st[i].ring_lo; r.nring = st[i].nring;
+        r.cc = (float)std::cos(st[i].lat); r.sc = (float)std::sin(st[i].lat);
+        r.pad_[0] = r.pad_[1] = r.pad_[2] = 0;
+    }
+    HCG_CUDA(c, c->d_rowsf.ensure(rows.size() * sizeof(RowF)));
+    HCG_CUDA(c, cudaMemcpy(c->d_rowsf.p, rows.data(), rows.size() * sizeof(RowF), cudaMemcpyHostToDevice));
+    c->dlmax = dlmax;
+    c->car_u0 = st[0].u0; c->car_du = st[0].du;
+    // the tile kernel walks a plate-carree target whose region is a plain longitude window
+    // (no wrap) with a per-ring table narrow enough for fp32 bin arithmetic
+    c->tile_ok = strip_cells > 1 && !rg.full_circle && c->f32_series_ok && rg.m < (1 << 22);
     const int threads = 128;
     const unsigned blocks = (unsigned)((nw + threads - 1) / threads);
     ring_window_kernel<<<blocks, threads>>>(c->d_strips.as<Strip>(), c->d_wins.as<RingWin>(),
-                                            (int)st.size(), kmax, rg, R);
+                                            c->d_winsf.as<RingWinF>(), (int)st.size(), kmax, rg, R);
     HCG_CUDA(c, cudaGetLastError());
     HCG_CUDA(c, cudaDeviceSynchronize());
     c->has_target = true;
@@ -207,6 +232,7 @@ int build_target_car(hcgrid_ctx* c, int nx, int ny, double lon0, double lat0, do
     const double a = lon0 * kDeg2Rad, b = (lon0 + span) * kDeg2Rad;
     c->is_car = true;
     c->ncell = (int64_t)nx * ny;
+    c->car_dlat = dlat * kDeg2Rad;
     return finish_target(c, hs, nx, std::min(a, b), std::max(a, b));
 }
 

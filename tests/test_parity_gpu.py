@@ -86,24 +86,71 @@ def test_config_miniature_f64(oracle, cfg):
 
 
 # ------------------------------------------------------------ every kernel variant / coarsening
+# stats()["kernel"] of each forced variant: simple 1, fp64 pair 4, general 3, staged 2, tile 6
+KERNEL_IDS = {1: 1, 2: 4, 3: 3, 4: 2, 5: 6}
+
+
 @pytest.mark.parametrize("cfg", [1, 3, 5])
-@pytest.mark.parametrize("kernel", [1, 2, 3])
+@pytest.mark.parametrize("kernel", [1, 2, 3, 4, 5])
 def test_kernel_variants(oracle, cfg, kernel):
     from paper_2012_13173_b200 import binding
     w, ref = mini(oracle, cfg)
     cube, wmap, cnt, st = run_gpu(w, "f32", {binding.OPT_KERNEL: kernel})
+    assert st["kernel"] == KERNEL_IDS[kernel]
     compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F32, qmax(w))
 
 
-@pytest.mark.parametrize("coarsen", [1, 2, 3, 4, 6, 8])
+def test_auto_kernel_is_the_tile_kernel_on_car_targets(oracle):
+    w, ref = mini(oracle, 3)
+    _, _, _, st = run_gpu(w, "f32")
+    assert st["kernel"] == 6 and st["coarsen"] * st["coarsen_y"] >= 2
+
+
+@pytest.mark.parametrize("coarsen", [1, 2, 4, 8])
 @pytest.mark.parametrize("cfg", [1, 5])
-def test_coarsening(oracle, cfg, coarsen):
+def test_coarsening_simple_and_staged(oracle, cfg, coarsen):
     from paper_2012_13173_b200 import binding
     w, ref = mini(oracle, cfg)
-    for kernel in (0, 1):
+    for kernel in (binding.KERNEL_SIMPLE, binding.KERNEL_STAGED):
         cube, wmap, cnt, st = run_gpu(w, "f32", {binding.OPT_COARSEN: coarsen, binding.OPT_KERNEL: kernel})
         assert st["coarsen"] == coarsen
         compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F32, qmax(w))
+
+
+TILE_SHAPES = [(1, 1), (2, 1), (4, 1), (8, 1), (2, 2), (4, 2), (8, 2), (4, 4)]
+
+
+@pytest.mark.parametrize("shape", TILE_SHAPES, ids=lambda s: f"{s[0]}x{s[1]}")
+@pytest.mark.parametrize("cfg", [1, 2, 3, 5])
+def test_tile_shapes(oracle, cfg, shape):
+    """Every built tile shape of the tile kernel, with and without the count output; the
+    miniature targets are not multiples of the tile, so ragged right / bottom tiles run too."""
+    from paper_2012_13173_b200 import binding
+    w, ref = mini(oracle, cfg)
+    opts = {binding.OPT_KERNEL: binding.KERNEL_TILE, binding.OPT_COARSEN: shape[0], binding.OPT_COARSEN_Y: shape[1]}
+    cube, wmap, cnt, st = run_gpu(w, "f32", opts)
+    assert (st["kernel"], st["coarsen"], st["coarsen_y"]) == (6, shape[0], shape[1])
+    compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F32, qmax(w))
+    cube2, wmap2, cnt2, _ = run_gpu(w, "f32", opts, want_counts=False)
+    assert cnt2 is None
+    compare(cube2, wmap2, None, ref, w.sigma_deg, w.radius_deg, TOL_F32, qmax(w))
+
+
+@pytest.mark.parametrize("radius_deg,sigma_deg", [(0.1, 0.04), (0.2, 0.08), (1.5, 0.5)])
+def test_tile_series_modes(oracle, radius_deg, sigma_deg):
+    """Wider kernels switch the tile kernel's pair arithmetic to the series / full modes."""
+    rng = np.random.default_rng(77)
+    n = 6000
+    w = workloads.make(1, 1.0)
+    w.lon = 200.0 + rng.uniform(-2.0, 2.0, n)
+    w.lat = 40.0 + rng.uniform(-2.0, 2.0, n)
+    w.values = rng.normal(size=(n, 1)).astype(np.float32)
+    w.sigma_deg, w.radius_deg, w.nside = sigma_deg, radius_deg, 256
+    w.target = workloads.CarTarget(23, 19, 199.0, 39.1, 0.09, 0.1)
+    ref = run_oracle(oracle, w)
+    cube, wmap, cnt, st = run_gpu(w, "f32")
+    assert st["kernel"] == 6
+    compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F32)
 
 
 @pytest.mark.parametrize("subpix", [0, 1, 3])
