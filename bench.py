@@ -279,7 +279,7 @@ def run_product(args):
     rl.update({
         "traffic": args.traffic,
         "kernel": {1: "conv1_simple_f32", 2: "conv1_staged_f32", 3: "conv_general<f32>", 4: "conv_general<f64 pair>",
-                   5: "conv_general<f64>"}.get(st["kernel"], str(st["kernel"])),
+                   5: "conv_general<f64>", 6: "conv1_tile_f32"}.get(st["kernel"], str(st["kernel"])),
         "kernel_us": t_conv * 1e6, "t_roof_us": mdl["t_roof_s"] * 1e6,
         "legs_us": {"fp32": mdl["t_fp32_s"] * 1e6, "mufu": mdl["t_mufu_s"] * 1e6, "hbm": mdl["t_hbm_s"] * 1e6},
         "n_hit": n_hit, "n_cand": cand["n_cand"], "n_cand_rows_counted": cand["rows_counted"],
@@ -314,7 +314,7 @@ def run_product(args):
                    "nchan": nchan, "nside": w.nside, "sigma_arcmin": w.sigma_deg * 60, "radius_arcmin": w.radius_deg * 60,
                    "l2": "inputs larger than L2 (no flush): lon/lat/values %.0f MB + packed records %.0f MB per step"
                          % (h2d / 1e6, st["n_kept"] * 16 / 1e6),
-                   "coarsen": st["coarsen"], "subpix_bits": st["subpix_bits"], "per_rank": "one independent problem"},
+                   "coarsen": st["coarsen"], "coarsen_y": st["coarsen_y"], "subpix_bits": st["subpix_bits"], "per_rank": "one independent problem"},
         "kernel_evals_per_s": n_hit * world * args.steps / (ms_total * 1e-3),
         "conv_kernel": {"us": t_conv * 1e6, "cell_channels_per_s": ncell * nchan / t_conv,
                         "kernel_evals_per_s": n_hit / t_conv},

@@ -50,6 +50,7 @@ struct TileConst {
     float cc0, p1, p2, p3;      // cos(lat_s) = cc0 + dy (p1 + dy (p2 + dy p3)), dy scaled
     float cc[GY];
     float a12, hmax;
+    float hm;                   // hmax, or -1 for a lane that is past the end of the stream
 };
 
 // MODE 0 "flat": d^2 = dy^2 + cos cos dx^2 (valid while R^2/12 and dl_max^2/12 < 1e-7);
@@ -66,13 +67,13 @@ __device__ __forceinline__ void tile_pairs(const uint4 raw, const TileConst<GY>&
     float V[GX], U[GY], C[GY];
 #pragma unroll
     for (int i = 0; i < GX; ++i) {
-        const float dx = fmaf(-(float)i, tc.duk, dx0);
+        const float dx = i == 0 ? dx0 : fmaf(-(float)i, tc.duk, dx0);
         const float v = dx * dx;
         V[i] = MODE >= 1 ? v * fmaf(v, -tc.a12, 1.0f) : v;
     }
 #pragma unroll
     for (int j = 0; j < GY; ++j) {
-        const float dy = fmaf(-(float)j, tc.dyk, dy0);
+        const float dy = j == 0 ? dy0 : fmaf(-(float)j, tc.dyk, dy0);
         const float u = dy * dy;
         U[j] = MODE >= 1 ? u * fmaf(u, -tc.a12, 1.0f) : u;
         C[j] = tc.cc[j] * cs;
@@ -84,7 +85,7 @@ __device__ __forceinline__ void tile_pairs(const uint4 raw, const TileConst<GY>&
             const float h = fmaf(C[j], V[i], U[j]);
             const float e = MODE == 2 ? h * fmaf(h, tc.a12, 1.0f) : h;
             const float w = ex2_approx(-e);
-            if (h <= tc.hmax) {
+            if (h <= tc.hm) {
                 W[j * GX + i] = fmaf(w, q, W[j * GX + i]);
                 S[j * GX + i] = fmaf(w, qv, S[j * GX + i]);
                 if (COUNTS) cnt[j * GX + i] += 1;
@@ -117,6 +118,24 @@ struct TileReduce {
     }
 };
 
+// ---- the candidate stream's ring cursor (step iv): entry k of the per-warp table is
+// (end position of ring k in the stream, record address of stream index 0 within ring k)
+__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void lds_entry(uint32_t tp, int& end, unsigned long long& base) {
+    unsigned long long e;
+    asm volatile("ld.shared.v2.u64 {%0, %1}, [%2];" : "=l"(e), "=l"(base) : "r"(tp));
+    end = (int)e;
+}
+__device__ __forceinline__ void stream_seek(int i, uint32_t& tp, int& end, unsigned long long& base) {
+    while (i >= end) {
+        tp += 16;
+        lds_entry(tp, end, base);
+    }
+}
+__device__ __forceinline__ uint4 ldg_rec(unsigned long long base, int i) {
+    return __ldg((const uint4*)(uintptr_t)(base + (unsigned long long)(unsigned)i * 16ull));
+}
+
 constexpr int ilog2(int n) { return n <= 1 ? 0 : 1 + ilog2(n / 2); }
 
 constexpr int kTileWarps = 4;
@@ -125,7 +144,7 @@ template <int GX, int GY, int MODE, bool COUNTS>
 __global__ void __launch_bounds__(kTileWarps * 32)
 conv1_tile_f32(const TileArgs a) {
     constexpr int NC = GX * GY;
-    __shared__ int2 s_tab[kTileWarps][32];
+    __shared__ ulonglong2 s_tab[kTileWarps][32];
     const int lane = threadIdx.x & 31;
     const int wib = threadIdx.x >> 5;
     const int64_t tile = (int64_t)blockIdx.x * kTileWarps + wib;
@@ -174,7 +193,7 @@ conv1_tile_f32(const TileArgs a) {
     const float fxw = (float)(a.du >= 0.0 ? ix0 : ix0 + ncols - 1);   // westmost / eastmost column of the tile
     const float fxe = (float)(a.du >= 0.0 ? ix0 + ncols - 1 : ix0);
     const Rec32* __restrict__ rec = a.rec;
-    int2* tab = s_tab[wib];
+    ulonglong2* tab = s_tab[wib];
 
     for (int rb = rmin; rb <= rmax; rb += 32) {
         // ---- steps (ii)+(iii): lane k <-> ring rb + k
@@ -210,27 +229,43 @@ conv1_tile_f32(const TileArgs a) {
         }
         const int total = __shfl_sync(0xffffffffu, incl, 31);
         __syncwarp();                                   // previous pass done with the table
-        tab[lane] = make_int2(incl, sa - (incl - sn)); // (end of ring k in the stream, address offset)
+        // (end of ring k in the stream, address of the record that would have stream index 0)
+        tab[lane] = make_ulonglong2((unsigned long long)(unsigned)incl,
+                                    (unsigned long long)(uintptr_t)(rec + ((long long)sa - (incl - sn))));
         __syncwarp();
+        if (total == 0) continue;
 
-        // ---- steps (iv)+(v): the candidate stream, one record ahead
+        // ---- steps (iv)+(v): the candidate stream, one record ahead in two named buffers.
+        // The trip count is warp-uniform; a lane past the end re-reads the last record and
+        // drops it by testing against a negative threshold.
+        const int last = total - 1;
+        const int niter = (total + 31) >> 5;
+        uint32_t tp = smem_addr(tab);                   // ring cursor: shared address of entry k
+        int end;
+        unsigned long long base;
+        lds_entry(tp, end, base);
         int i = lane;
-        if (i < total) {
-            int k = 0;
-            int2 t = tab[0];
-            while (i >= t.x) t = tab[++k];
-            uint4 nxt = __ldg((const uint4*)(rec + (t.y + i)));
-            while (true) {
-                const uint4 cur = nxt;
-                const int i2 = i + 32;
-                const bool more = i2 < total;
-                if (more) {
-                    while (i2 >= t.x) t = tab[++k];
-                    nxt = __ldg((const uint4*)(rec + (t.y + i2)));
-                }
-                tile_pairs<GX, GY, MODE, COUNTS>(cur, tc, W, S, cnt);
-                if (!more) break;
-                i = i2;
+        stream_seek(min(i, last), tp, end, base);
+        uint4 ra = ldg_rec(base, min(i, last));
+        for (int it = 0; it < niter; it += 2) {
+            const int i1 = i + 32;
+            {
+                const int ii = min(i1, last);
+                stream_seek(ii, tp, end, base);
+                const uint4 rb = ldg_rec(base, ii);
+                tc.hm = i <= last ? tc.hmax : -1.0f;
+                tile_pairs<GX, GY, MODE, COUNTS>(ra, tc, W, S, cnt);
+                ra = rb;
+            }
+            if (it + 1 >= niter) break;
+            i += 64;
+            {
+                const int ii = min(i, last);
+                stream_seek(ii, tp, end, base);
+                const uint4 rb = ldg_rec(base, ii);
+                tc.hm = i1 <= last ? tc.hmax : -1.0f;
+                tile_pairs<GX, GY, MODE, COUNTS>(ra, tc, W, S, cnt);
+                ra = rb;
             }
         }
     }
@@ -281,7 +316,9 @@ static double shape_cost(int gx, int gy, int mode, bool counts, double cw, doubl
                             (5.0 + (counts ? 1.0 : 0.0) + (mode == 2 ? 2.0 : 0.0)) * gx * gy;
     const double iters = cand_per_cell * infl / 32.0 + 0.5;
     const double overhead = 150.0 + 14.0 * gy + 8.0 * gx * gy;
-    return (iters * per_iter + overhead) / (gx * gy);
+    // 16-cell tiles need ~100 registers per thread; the lower occupancy cost ~12 % on B200
+    const double occ = gx * gy >= 16 ? 1.12 : 1.0;
+    return occ * (iters * per_iter + overhead) / (gx * gy);
 }
 
 int launch_conv_tile(hcgrid_ctx* c, int64_t n, float* cube, float* wmap, int32_t* counts, cudaStream_t st) {
