@@ -60,7 +60,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
@@ -180,9 +180,11 @@ def run_product(args):
     val = torch.from_numpy(w.values).to(dev)
     wts = None if w.weights is None else torch.from_numpy(w.weights).to(dev)
     ncell, nchan = t.ncell, w.nchan
+    # the timed call returns what the north_star names: datacube and weight map.  The optional
+    # contributing-sample counts (a parity output) are fetched by one extra, untimed call.
+    cnt_t = torch.empty(ncell, dtype=torch.int32, device=dev)
     out = (torch.empty((ncell, nchan), dtype=torch.float32, device=dev),
-           torch.empty(ncell, dtype=torch.float32, device=dev),
-           torch.empty(ncell, dtype=torch.int32, device=dev))
+           torch.empty(ncell, dtype=torch.float32, device=dev), None)
 
     def barrier():
         if world > 1:
@@ -190,7 +192,7 @@ def run_product(args):
         torch.cuda.synchronize()
 
     def step():
-        g.grid(lon, lat, val, wts, out=out)
+        g.grid(lon, lat, val, wts, want_counts=False, out=out)
 
     for _ in range(max(args.warmup, 3)):
         step()
@@ -219,22 +221,25 @@ def run_product(args):
         s = g.stats()
         for k in stage:
             stage[k].append(s[k])
-    g.set_option(binding.OPT_PROFILE, 0)
     st = g.stats()
-    clocks = sampler.stop() if rank == 0 else None
+    # the same call with the count output (untimed for `value`; its convolution time is reported)
+    us_conv_counts = []
+    for _ in range(3):
+        g.grid(lon, lat, val, wts, want_counts=True, out=(out[0], out[1], cnt_t))
+        us_conv_counts.append(g.stats()["us_convolve"])
+    g.set_option(binding.OPT_PROFILE, 0)
 
     # ---- timed region 3: end to end through hcgrid_grid_host, pinned host buffers
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     h_lon, h_lat, h_val = pin(w.lon), pin(w.lat), pin(w.values)
     h_wts = None if w.weights is None else pin(w.weights)
     h_out = (torch.empty((ncell, nchan), dtype=torch.float32).pin_memory(),
-             torch.empty(ncell, dtype=torch.float32).pin_memory(),
-             torch.empty(ncell, dtype=torch.int32).pin_memory())
-    h_out_np = tuple(x.numpy() for x in h_out)
+             torch.empty(ncell, dtype=torch.float32).pin_memory())
+    h_out_np = tuple(x.numpy() for x in h_out) + (None,)
 
     def step_host():
         g.grid_host(h_lon.numpy(), h_lat.numpy(), h_val.numpy(), None if h_wts is None else h_wts.numpy(),
-                    out=h_out_np)
+                    want_counts=False, out=h_out_np)
 
     for _ in range(2):
         step_host()
@@ -245,15 +250,16 @@ def run_product(args):
     e1.record()
     barrier()
     ms_e2e = e0.elapsed_time(e1)
+    clocks = sampler.stop() if rank == 0 else None
     h2d = w.n * (16 + 4 * nchan + (4 if w.weights is not None else 0))
-    d2h = ncell * (4 * nchan + 8)
+    d2h = ncell * (4 * nchan + 4)
 
     # ---- max over ranks
     if world > 1:
         tmax = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device=dev)
         dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
         ms_total, ms_e2e = float(tmax[0]), float(tmax[1])
-    cnt = out[2].cpu().numpy().astype(np.int64)
+    cnt = cnt_t.cpu().numpy().astype(np.int64)
     n_hit = int(cnt.sum())
     if rank != 0:
         if world > 1:
@@ -266,7 +272,8 @@ def run_product(args):
     t_conv = float(np.mean(stage["us_convolve"])) * 1e-6
     cand = roofline.count_candidates(w, max_rows=args.cand_rows)
     p_fp32_meas, p_mufu_meas = binding.measure_peaks(local)
-    mdl = roofline.model(w.n, ncell, nchan, w.weights is not None, n_hit, cand["n_cand"], hbm_gbs)
+    mdl = roofline.model(w.n, ncell, nchan, w.weights is not None, n_hit, cand["n_cand"], hbm_gbs,
+                         want_counts=False)
     if mdl["bound"] == "hbm":
         rl = {"bound": "hbm", "achieved": mdl["bytes_unique"] / t_conv / 1e9, "peak": hbm_gbs, "unit": "GB/s"}
     elif mdl["bound"] == "mufu":
@@ -314,10 +321,12 @@ def run_product(args):
                    "nchan": nchan, "nside": w.nside, "sigma_arcmin": w.sigma_deg * 60, "radius_arcmin": w.radius_deg * 60,
                    "l2": "inputs larger than L2 (no flush): lon/lat/values %.0f MB + packed records %.0f MB per step"
                          % (h2d / 1e6, st["n_kept"] * 16 / 1e6),
-                   "coarsen": st["coarsen"], "coarsen_y": st["coarsen_y"], "subpix_bits": st["subpix_bits"], "per_rank": "one independent problem"},
+                   "coarsen": st["coarsen"], "coarsen_y": st["coarsen_y"], "subpix_bits": st["subpix_bits"], "per_rank": "one independent problem",
+                   "outputs": "datacube + weight map (count output off in the timed calls)"},
         "kernel_evals_per_s": n_hit * world * args.steps / (ms_total * 1e-3),
         "conv_kernel": {"us": t_conv * 1e6, "cell_channels_per_s": ncell * nchan / t_conv,
-                        "kernel_evals_per_s": n_hit / t_conv},
+                        "kernel_evals_per_s": n_hit / t_conv,
+                        "us_with_count_output": float(np.median(us_conv_counts))},
         "stages_us": {k[3:]: float(np.mean(v)) for k, v in stage.items()},
         "roofline": rl,
         "cpu_baseline": cpu,
@@ -336,7 +345,7 @@ def run_product(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="product", choices=["product", "reference"])
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])

@@ -85,10 +85,18 @@ __device__ __forceinline__ void tile_pairs(const uint4 raw, const TileConst<GY>&
             const float h = fmaf(C[j], V[i], U[j]);
             const float e = MODE == 2 ? h * fmaf(h, tc.a12, 1.0f) : h;
             const float w = ex2_approx(-e);
-            if (h <= tc.hm) {
+            // predicated accumulate, spelled out so the count stays one predicated add
+            if (COUNTS)
+                asm("{\n\t.reg .pred p;\n\t"
+                    "setp.le.f32 p, %3, %4;\n\t"
+                    "@p fma.rn.f32 %0, %5, %6, %0;\n\t"
+                    "@p fma.rn.f32 %1, %5, %7, %1;\n\t"
+                    "@p add.s32 %2, %2, 1;\n\t}"
+                    : "+f"(W[j * GX + i]), "+f"(S[j * GX + i]), "+r"(cnt[j * GX + i])
+                    : "f"(h), "f"(tc.hm), "f"(w), "f"(q), "f"(qv));
+            else if (h <= tc.hm) {
                 W[j * GX + i] = fmaf(w, q, W[j * GX + i]);
                 S[j * GX + i] = fmaf(w, qv, S[j * GX + i]);
-                if (COUNTS) cnt[j * GX + i] += 1;
             }
         }
     }
@@ -121,13 +129,17 @@ struct TileReduce {
 // ---- the candidate stream's ring cursor (step iv): entry k of the per-warp table is
 // (end position of ring k in the stream, record address of stream index 0 within ring k)
 __device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void lds_entry(uint32_t tp, int& end, unsigned long long& base) {
-    unsigned long long e;
-    asm volatile("ld.shared.v2.u64 {%0, %1}, [%2];" : "=l"(e), "=l"(base) : "r"(tp));
-    end = (int)e;
+__device__ __forceinline__ void lds_entry(uint32_t tp, unsigned long long& end, unsigned long long& base) {
+    asm volatile("ld.shared.v2.u64 {%0, %1}, [%2];" : "=l"(end), "=l"(base) : "r"(tp));
 }
-__device__ __forceinline__ void stream_seek(int i, uint32_t& tp, int& end, unsigned long long& base) {
-    while (i >= end) {
+__device__ __forceinline__ void stream_seek(int i, uint32_t& tp, unsigned long long& end, unsigned long long& base) {
+    // a step of 32 usually crosses one ring boundary: one predicated advance, then the loop
+    asm volatile("{\n\t.reg .pred p;\n\t"
+                 "setp.ge.s32 p, %3, %4;\n\t"
+                 "@p add.u32 %2, %2, 16;\n\t"
+                 "@p ld.shared.v2.u64 {%0, %1}, [%2];\n\t}"
+                 : "+l"(end), "+l"(base), "+r"(tp) : "r"(i), "r"((int)end));
+    while (i >= (int)end) {
         tp += 16;
         lds_entry(tp, end, base);
     }
@@ -147,10 +159,10 @@ conv1_tile_f32(const TileArgs a) {
     __shared__ ulonglong2 s_tab[kTileWarps][32];
     const int lane = threadIdx.x & 31;
     const int wib = threadIdx.x >> 5;
-    const int64_t tile = (int64_t)blockIdx.x * kTileWarps + wib;
-    if (tile >= a.ntiles) return;
-    const int ty = (int)(tile / a.tiles_x);
-    const int ix0 = (int)(tile - (int64_t)ty * a.tiles_x) * GX;
+    const unsigned tile = blockIdx.x * kTileWarps + wib;         // ntiles <= 2^30 (api.cu)
+    if (tile >= (unsigned)a.ntiles) return;
+    const int ty = (int)(tile / (unsigned)a.tiles_x);
+    const int ix0 = (int)(tile - (unsigned)ty * (unsigned)a.tiles_x) * GX;
     const int row0 = ty * GY;
     const int ncols = min(GX, a.nx - ix0);
     const int nrows = min(GY, a.ny - row0);
@@ -241,8 +253,7 @@ conv1_tile_f32(const TileArgs a) {
         const int last = total - 1;
         const int niter = (total + 31) >> 5;
         uint32_t tp = smem_addr(tab);                   // ring cursor: shared address of entry k
-        int end;
-        unsigned long long base;
+        unsigned long long end, base;
         lds_entry(tp, end, base);
         int i = lane;
         stream_seek(min(i, last), tp, end, base);

@@ -11,7 +11,8 @@ Definitions:
           production kernel's loops (whatever windows the kernel really walks, it is
           credited with these pairs only).
   T_roof = max( (N_cand F_d + N_hit F_a) / P_fp32 ,  N_hit / P_mufu ,  B_unique / BW_hbm )
-  F_d = 12 FP32-pipe instructions per candidate, F_a = 6 + nchan (+1 with weights) per hit,
+  F_d = 12 FP32-pipe instructions per candidate, F_a = 5 + nchan (+1 with weights, +1 with the
+  count output) per hit,
   one MUFU.EX2 per hit; B_unique = the API-level arrays once each.
 
 Nothing here runs on the product path; the pixel indices come from the library's own
@@ -33,8 +34,10 @@ P_FP32_NOMINAL = NUM_SMS * FP32_LANES_PER_SM * SM_MAX_HZ
 P_MUFU_NOMINAL = NUM_SMS * MUFU_LANES_PER_SM * SM_MAX_HZ
 
 
-def f_a(nchan: int, has_weights: bool) -> int:
-    return 6 + nchan + (1 if has_weights else 0)
+def f_a(nchan: int, has_weights: bool, want_counts: bool = True) -> int:
+    """FP32-pipe instructions per accepted pair; the count increment is only charged when the
+    count output is requested."""
+    return 5 + nchan + (1 if has_weights else 0) + (1 if want_counts else 0)
 
 
 def _ring_z(nside: int) -> np.ndarray:
@@ -129,7 +132,7 @@ def count_candidates(w, max_rows: int | None = None) -> dict:
 def model(n: int, ncell: int, nchan: int, has_weights: bool, n_hit: int, n_cand: int, hbm_gbs: float,
           p_fp32: float = P_FP32_NOMINAL, p_mufu: float = P_MUFU_NOMINAL, want_counts: bool = True) -> dict:
     """The three legs of T_roof in seconds and which one binds."""
-    inst = n_cand * F_D + n_hit * f_a(nchan, has_weights)
+    inst = n_cand * F_D + n_hit * f_a(nchan, has_weights, want_counts)
     b_unique = n * (16 + 4 * nchan + (4 if has_weights else 0)) + ncell * (4 * nchan + 4 + (4 if want_counts else 0))
     t_fp32 = inst / p_fp32
     t_mufu = n_hit / p_mufu
