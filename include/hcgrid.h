@@ -64,7 +64,8 @@ enum {
                                     2 = force the fp64 pair arithmetic with the F32 output type;
                                     3 = force the general (any nchan) kernel with fp32 pair arithmetic;
                                     4 = force the TMA-staged single-channel kernel;
-                                    5 = force the tile kernel (error if the target does not allow it) */
+                                    5 = force the tile kernel (error if the target does not allow it);
+                                    6 = force the cube kernel (nchan > 1; error if not applicable) */
     HCGRID_OPT_WARPS_PER_SM = 5, /* resident convolution warps per SM (staged kernel); 0 = auto */
     HCGRID_OPT_COARSEN_Y = 6     /* target rows per warp task (tile kernel); 0 = auto */
 };

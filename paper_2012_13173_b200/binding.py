@@ -19,7 +19,7 @@ _lib = None
 
 F32, F64 = 0, 1
 OPT_PROFILE, OPT_SUBPIX_BITS, OPT_COARSEN, OPT_KERNEL, OPT_WARPS_PER_SM, OPT_COARSEN_Y = 1, 2, 3, 4, 5, 6
-KERNEL_AUTO, KERNEL_SIMPLE, KERNEL_F64PAIR, KERNEL_GENERAL, KERNEL_STAGED, KERNEL_TILE = 0, 1, 2, 3, 4, 5
+KERNEL_AUTO, KERNEL_SIMPLE, KERNEL_F64PAIR, KERNEL_GENERAL, KERNEL_STAGED, KERNEL_TILE, KERNEL_CUBE = 0, 1, 2, 3, 4, 5, 6
 
 EXPORTS = [
     "hcgrid_create", "hcgrid_destroy", "hcgrid_set_option", "hcgrid_set_target_car",

@@ -105,7 +105,7 @@ int hcgrid_set_option(hcgrid_ctx* c, int option, int64_t value) {
             c->opt_coarsen = (int)value;
             break;
         case HCGRID_OPT_KERNEL:
-            if (value < 0 || value > 5) return fail(c, HCGRID_ERR_INVALID_ARG, "kernel must be 0..5");
+            if (value < 0 || value > 6) return fail(c, HCGRID_ERR_INVALID_ARG, "kernel must be 0..6");
             c->opt_kernel = (int)value;
             break;
         case HCGRID_OPT_COARSEN_Y:

@@ -303,7 +303,14 @@ int run_convolve(hcgrid_ctx* c, int64_t n, const float* values, int nchan, bool 
     if (c->opt_kernel == 5 && !(f32 && nchan == 1 && c->tile_ok))
         return fail(c, HCGRID_ERR_UNSUPPORTED, "the tile kernel needs fp32 mode, one channel and a plate-carree "
                     "target whose reach is a plain longitude window");
-    if (f32 && nchan == 1 && c->tile_ok && (c->opt_kernel == 0 || c->opt_kernel == 5)) {
+    const bool mc_ok = f32 && nchan > 1 && c->tile_ok && nchan % 4 == 0 && ((uintptr_t)values & 15) == 0;
+    if (c->opt_kernel == 6 && !mc_ok)
+        return fail(c, HCGRID_ERR_UNSUPPORTED, "the cube kernel needs fp32 mode, nchan a multiple of 4 (> 1), 16-byte "
+                    "aligned values and a plate-carree target whose reach is a plain longitude window");
+    if (mc_ok && (c->opt_kernel == 0 || c->opt_kernel == 6)) {
+        rc = launch_conv_mc(c, values, nchan, (float*)cube, (float*)wmap, counts, st);
+        c->stats.kernel = 7;
+    } else if (f32 && nchan == 1 && c->tile_ok && (c->opt_kernel == 0 || c->opt_kernel == 5)) {
         rc = launch_conv_tile(c, n, (float*)cube, (float*)wmap, counts, st);
         c->stats.kernel = 6;
     } else if (f32 && nchan == 1 && c->opt_kernel != 3) {

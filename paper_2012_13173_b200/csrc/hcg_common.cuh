@@ -92,6 +92,7 @@ struct Region {            // what of the sphere the target can reach (host + de
     double lat_lo;         // rad
     double wy;             // rad, latitude extent mapped onto 2^32
     int64_t nbins;         // nring * m
+    double sx32, sy32;     // fixed-point units per radian: 2^32 / wx, 2^32 / wy
 };
 
 struct KernelParams {      // per-context constants of the pair arithmetic

@@ -91,6 +91,10 @@ __device__ __forceinline__ bool pair32(const Rec32& r, const TaskConst& tc, floa
 // launcher of convolve_tile.cu (single channel, fp32, plate-carree targets)
 int launch_conv_tile(hcgrid_ctx* c, int64_t n, float* cube, float* wmap, int32_t* counts, cudaStream_t st);
 
+// launcher of convolve_mc.cu (many channels, fp32, plate-carree targets, nchan % 4 == 0)
+int launch_conv_mc(hcgrid_ctx* c, const float* values, int nchan, float* cube, float* wmap, int32_t* counts,
+                   cudaStream_t st);
+
 // launcher of convolve_gen.cu
 int launch_conv_general(hcgrid_ctx* c, const ConvArgs& a, bool pair_f64, bool out_double, cudaStream_t st);
 

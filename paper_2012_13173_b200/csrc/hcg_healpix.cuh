@@ -29,6 +29,8 @@ constexpr double kTwoPi = 6.28318530717958647692;
 constexpr double kHalfPi = 1.57079632679489661923;
 constexpr double kDeg2Rad = kPi / 180.0;
 constexpr double kSqrt6 = 2.44948974278317809820;
+constexpr double kInvTwoPi = 0.15915494309189533577;
+constexpr double kInvHalfPi = 0.63661977236758134308;
 
 // pixels in ring `iring` (1 .. 4 nside - 1)
 HCG_HD int ring_npix(int iring, int nside) {
@@ -79,7 +81,7 @@ HCG_HD void ang2ring(int nside, double lon, double lat, int& iring, int& ip) {
     const double n = (double)nside;
     const double z = sin(lat);
     const double za = fabs(z);
-    double tt = lon / kHalfPi;                     // [0, 4)
+    double tt = lon * kInvHalfPi;                  // [0, 4)
     if (tt >= 4.0) tt -= 4.0;
     if (tt < 0.0) tt = 0.0;
     if (za <= 2.0 / 3.0) {                         // equatorial belt
@@ -97,7 +99,7 @@ HCG_HD void ang2ring(int nside, double lon, double lat, int& iring, int& ip) {
     } else {                                       // polar caps
         const double tp = tt - floor(tt);
         const double sh = sin(0.5 * (kHalfPi - fabs(lat)));
-        const double tmp = n * sqrt(6.0) * sh;     // n sqrt(3 (1 - |z|)), 1-|z| = 2 sin^2(colat/2)
+        const double tmp = n * kSqrt6 * sh;     // n sqrt(3 (1 - |z|)), 1-|z| = 2 sin^2(colat/2)
         long long jp = (long long)(tp * tmp);
         long long jm = (long long)((1.0 - tp) * tmp);
         long long ir = jp + jm + 1;                // ring counted from the closest pole
@@ -115,7 +117,7 @@ HCG_HD void ang2ring(int nside, double lon, double lat, int& iring, int& ip) {
 HCG_HD long long ring_bin(int iring, int nside, int ip, double lon, int b) {
     if (b <= 0) return (long long)(ip >> (-b));
     const int npr = ring_npix(iring, nside);
-    const double g = lon * ((double)npr / kTwoPi) + ring_off(iring, nside);
+    const double g = lon * ((double)npr * kInvTwoPi) + ring_off(iring, nside);
     double d = g - (double)ip;
     if (d > 0.5 * npr) d -= npr;
     if (d < -0.5 * npr) d += npr;
@@ -135,7 +137,7 @@ HCG_HD long long ring_nbins(int iring, int nside, int b) {
 // point sitting at the ring's centre latitude
 HCG_HD double ring_bin_coord(int iring, int nside, double lon, int b) {
     const int npr = ring_npix(iring, nside);
-    const double g = lon * ((double)npr / kTwoPi) + ring_off(iring, nside);
+    const double g = lon * ((double)npr * kInvTwoPi) + ring_off(iring, nside);
     return ldexp(g, b);
 }
 

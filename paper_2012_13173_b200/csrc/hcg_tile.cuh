@@ -1,0 +1,140 @@
+// hcg_tile.cuh -- what the tile kernels (convolve_tile.cu: one channel; convolve_mc.cu: many
+// channels) share: the argument block, the scaled fp32 pair arithmetic of step (v), the
+// candidate stream's ring cursor of step (iv) and the transposed warp reduction.
+#pragma once
+#include "hcg_conv.cuh"
+
+namespace hcg {
+
+struct TileArgs {
+    const RowF* rows;
+    const RingWinF* wins;
+    const int32_t* bin_start;
+    const Rec32* rec;
+    float* cube;
+    float* wmap;
+    int32_t* counts;
+    double u0, du, sx;          // lon offset of column 0 (rad), column step (rad), fixed-point units per rad
+    int32_t nx, ny, kmax, m;    // target shape, window-table row length, lookup bins per ring
+    int32_t tiles_x;
+    int64_t ntiles;
+    float sxk, syk;             // sqrt(kappa) * radians per fixed-point unit (lon, lat)
+    float duk, dyk;             // sqrt(kappa) * column step / row step (signed)
+    float isk;                  // 1 / sqrt(kappa)
+    float a12;                  // 1 / (12 kappa): series coefficient in scaled units
+    float hmax;                 // kappa * 4 sin^2(R/2)  (series modes)  or  kappa * R^2 (flat mode)
+};
+
+template <int GY>
+struct TileConst {
+    uint32_t xc0, yc0;
+    float sxk, syk, duk, dyk;
+    float cc0, p1, p2, p3;      // cos(lat_s) = cc0 + dy (p1 + dy (p2 + dy p3)), dy scaled
+    float cc[GY];
+    float a12, hmax;
+    float hm;                   // hmax, or -1 for a lane that is past the end of the stream
+};
+
+// MODE 0 "flat": d^2 = dy^2 + cos cos dx^2 (valid while R^2/12 and dl_max^2/12 < 1e-7);
+// MODE 1 "series": 4 hav(d) = u(1-u/12) + C v(1-v/12) for the test, weight from the same;
+// MODE 2 "full": as 1, plus d^2 = h(1 + h/12) for the weight.
+template <int GX, int GY, int MODE, bool COUNTS>
+__device__ __forceinline__ void tile_pairs(const uint4 raw, const TileConst<GY>& tc, float (&W)[GX * GY],
+                                           float (&S)[GX * GY], int (&cnt)[GX * GY]) {
+    const float q = __uint_as_float(raw.w);
+    const float qv = q * __uint_as_float(raw.z);
+    const float dx0 = (float)(int)(raw.x - tc.xc0) * tc.sxk;
+    const float dy0 = (float)(int)(raw.y - tc.yc0) * tc.syk;
+    const float cs = fmaf(dy0, fmaf(dy0, fmaf(dy0, tc.p3, tc.p2), tc.p1), tc.cc0);
+    float V[GX], U[GY], C[GY];
+#pragma unroll
+    for (int i = 0; i < GX; ++i) {
+        const float dx = i == 0 ? dx0 : fmaf(-(float)i, tc.duk, dx0);
+        const float v = dx * dx;
+        V[i] = MODE >= 1 ? v * fmaf(v, -tc.a12, 1.0f) : v;
+    }
+#pragma unroll
+    for (int j = 0; j < GY; ++j) {
+        const float dy = j == 0 ? dy0 : fmaf(-(float)j, tc.dyk, dy0);
+        const float u = dy * dy;
+        U[j] = MODE >= 1 ? u * fmaf(u, -tc.a12, 1.0f) : u;
+        C[j] = tc.cc[j] * cs;
+    }
+#pragma unroll
+    for (int j = 0; j < GY; ++j) {
+#pragma unroll
+        for (int i = 0; i < GX; ++i) {
+            const float h = fmaf(C[j], V[i], U[j]);
+            const float e = MODE == 2 ? h * fmaf(h, tc.a12, 1.0f) : h;
+            const float w = ex2_approx(-e);
+            // predicated accumulate, spelled out so the count stays one predicated add
+            if (COUNTS)
+                asm("{\n\t.reg .pred p;\n\t"
+                    "setp.le.f32 p, %3, %4;\n\t"
+                    "@p fma.rn.f32 %0, %5, %6, %0;\n\t"
+                    "@p fma.rn.f32 %1, %5, %7, %1;\n\t"
+                    "@p add.s32 %2, %2, 1;\n\t}"
+                    : "+f"(W[j * GX + i]), "+f"(S[j * GX + i]), "+r"(cnt[j * GX + i])
+                    : "f"(h), "f"(tc.hm), "f"(w), "f"(q), "f"(qv));
+            else if (h <= tc.hm) {
+                W[j * GX + i] = fmaf(w, q, W[j * GX + i]);
+                S[j * GX + i] = fmaf(w, qv, S[j * GX + i]);
+            }
+        }
+    }
+}
+
+// Transposed warp reduction of N (a power of two <= 32) per-lane values: after the call
+// v[0] of lane L holds the sum over all 32 lanes of value number L >> (5 - log2 N).
+template <int N, int SH, typename T>
+struct TileReduce {
+    static __device__ __forceinline__ void run(T* v, int lane) {
+        if constexpr (SH >= 1) {
+            if constexpr (N > 1) {
+                constexpr int H = N / 2;
+                const bool up = (lane & SH) != 0;
+#pragma unroll
+                for (int i = 0; i < H; ++i) {
+                    const T keep = up ? v[i + H] : v[i];
+                    const T send = up ? v[i] : v[i + H];
+                    v[i] = keep + __shfl_xor_sync(0xffffffffu, send, SH);
+                }
+                TileReduce<H, SH / 2, T>::run(v, lane);
+            } else {
+                v[0] += __shfl_xor_sync(0xffffffffu, v[0], SH);
+                TileReduce<1, SH / 2, T>::run(v, lane);
+            }
+        }
+    }
+};
+
+// ---- the candidate stream's ring cursor (step iv): entry k of the per-warp table is
+// (end position of ring k in the stream, record address of stream index 0 within ring k)
+__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void lds_entry(uint32_t tp, unsigned long long& end, unsigned long long& base) {
+    asm volatile("ld.shared.v2.u64 {%0, %1}, [%2];" : "=l"(end), "=l"(base) : "r"(tp));
+}
+__device__ __forceinline__ void stream_seek(int i, uint32_t& tp, unsigned long long& end, unsigned long long& base) {
+    // a step of 32 usually crosses one ring boundary: one predicated advance, then the loop
+    asm volatile("{\n\t.reg .pred p;\n\t"
+                 "setp.ge.s32 p, %3, %4;\n\t"
+                 "@p add.u32 %2, %2, 16;\n\t"
+                 "@p ld.shared.v2.u64 {%0, %1}, [%2];\n\t}"
+                 : "+l"(end), "+l"(base), "+r"(tp) : "r"(i), "r"((int)end));
+    while (i >= (int)end) {
+        tp += 16;
+        lds_entry(tp, end, base);
+    }
+}
+__device__ __forceinline__ uint4 ldg_rec(unsigned long long base, int i) {
+    return __ldg((const uint4*)(uintptr_t)(base + (unsigned long long)(unsigned)i * 16ull));
+}
+
+constexpr int ilog2(int n) { return n <= 1 ? 0 : 1 + ilog2(n / 2); }
+
+// Host side: the fields of TileArgs that depend only on the context (not on the tile shape
+// or the outputs), and the series mode the tolerances need.
+int tile_series_mode(const hcgrid_ctx* c);
+void fill_tile_args(const hcgrid_ctx* c, int mode, TileArgs& a);
+
+}  // namespace hcg

@@ -33,7 +33,8 @@ pixelise_kernel(const double* __restrict__ lon_deg, const double* __restrict__ l
     Rec32 r;
     r.xi = 0; r.yi = 0; r.idx = (uint32_t)i; r.q = 1.0f;
     if (isfinite(lo_d) && la_d >= -90.0 && la_d <= 90.0) {
-        double l = fmod(lo_d, 360.0);
+        double l = lo_d - 360.0 * floor(lo_d * (1.0 / 360.0));     // lon mod 360
+        if (l >= 360.0) l -= 360.0;
         if (l < 0.0) l += 360.0;
         const double lon = l * kDeg2Rad, lat = la_d * kDeg2Rad;
         int iring, ip;
@@ -43,16 +44,17 @@ pixelise_kernel(const double* __restrict__ lon_deg, const double* __restrict__ l
         if (u < 0.0) u += kTwoPi;
         if (u >= kTwoPi) u -= kTwoPi;
         if (rr >= 0 && rr < rg.nring && (rg.full_circle || u < rg.wx * (1.0 - 1e-9))) {
-            const long long bin = ring_bin(iring, rg.nside, ip, lon, rg.subpix);
-            const long long nb = ring_nbins(iring, rg.nside, rg.subpix);
-            const long long j0 = (long long)floor(ring_bin_coord(iring, rg.nside, rg.lon_lo, rg.subpix)) - 2;
-            long long jrel = (bin - j0) % nb;
+            const int bin = (int)ring_bin(iring, rg.nside, ip, lon, rg.subpix);
+            const int nb = (int)ring_nbins(iring, rg.nside, rg.subpix);
+            const int j0 = (int)floor(ring_bin_coord(iring, rg.nside, rg.lon_lo, rg.subpix)) - 2;   // in [-2, nb)
+            int jrel = bin - j0;                                     // in (-nb, nb + 2]
             if (jrel < 0) jrel += nb;
+            if (jrel >= nb) jrel -= nb;
             if (jrel < rg.m) {
-                key = (uint32_t)((long long)rr * rg.m + jrel);
+                key = (uint32_t)(rr * rg.m + jrel);
                 if (kF32) {
-                    r.xi = (uint32_t)(unsigned long long)llrint(u * (4294967296.0 / rg.wx));
-                    r.yi = (uint32_t)(unsigned long long)llrint((lat - rg.lat_lo) * (4294967296.0 / rg.wy));
+                    r.xi = (uint32_t)(unsigned long long)__double2ll_rn(u * rg.sx32);
+                    r.yi = (uint32_t)(unsigned long long)__double2ll_rn((lat - rg.lat_lo) * rg.sy32);
                 }
             }
         }
@@ -66,25 +68,43 @@ pixelise_kernel(const double* __restrict__ lon_deg, const double* __restrict__ l
     }
 }
 
+// a4 + a5 (fp32 mode) in one pass over the sorted pairs.
 // a4: bin_start from the sorted keys.  Thread i owns the gap (key[i-1], key[i]]; thread n
-// closes the table.  No atomics, every entry written exactly once.
+// closes the table.  Short gaps are written by their thread; long ones (ring boundaries,
+// the empty head and tail of the table) are queued in shared memory and filled by the whole
+// block.  Every entry is written exactly once, no global atomics.
+// a5: rec_out[i] = rec_in[sidx[i]] for the kept samples (rec_in == nullptr: tables only).
 __global__ void __launch_bounds__(256)
-bin_start_kernel(const uint32_t* __restrict__ skeys, int64_t n, int64_t nbins,
-                 int32_t* __restrict__ bin_start) {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i > n) return;
-    const int64_t prev = i == 0 ? -1 : (int64_t)skeys[i - 1];
-    const int64_t cur = i == n ? nbins : (int64_t)skeys[i];
-    for (int64_t k = prev + 1; k <= cur; ++k) bin_start[k] = (int32_t)i;
-}
-
-__global__ void __launch_bounds__(256)
-pack32_kernel(const uint32_t* __restrict__ skeys, const uint32_t* __restrict__ sidx, int64_t n,
-              uint32_t sentinel, const Rec32* __restrict__ rec_in, Rec32* __restrict__ rec_out) {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    if (skeys[i] == sentinel) return;
-    rec_out[i] = rec_in[sidx[i]];
+tables_pack_kernel(const uint32_t* __restrict__ skeys, const uint32_t* __restrict__ sidx, int64_t n,
+                   int32_t nbins, int32_t* __restrict__ bin_start, const Rec32* __restrict__ rec_in,
+                   Rec32* __restrict__ rec_out) {
+    __shared__ int s_cnt;
+    __shared__ int s_lo[256], s_hi[256], s_val[256];
+    const int tid = threadIdx.x;
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + tid;
+    if (tid == 0) s_cnt = 0;
+    __syncthreads();
+    uint4 rec = make_uint4(0, 0, 0, 0);
+    bool kept = false;
+    if (i <= n) {
+        const int prev = i == 0 ? -1 : (int)min(skeys[i - 1], (uint32_t)nbins);
+        const int cur = i == n ? nbins : (int)min(skeys[i], (uint32_t)nbins);
+        kept = rec_in != nullptr && i < n && cur != nbins;
+        if (kept) rec = __ldg((const uint4*)(rec_in + sidx[i]));
+        if (cur - prev <= 4) {
+            for (int k = prev + 1; k <= cur; ++k) bin_start[k] = (int32_t)i;
+        } else {
+            const int slot = atomicAdd(&s_cnt, 1);          // shared-memory queue slot, order irrelevant
+            s_lo[slot] = prev + 1; s_hi[slot] = cur; s_val[slot] = (int32_t)i;
+        }
+    }
+    if (kept) *(uint4*)(rec_out + i) = rec;
+    __syncthreads();
+    const int ngap = s_cnt;
+    for (int g = 0; g < ngap; ++g) {
+        const int hi = s_hi[g], val = s_val[g];
+        for (int k = s_lo[g] + tid; k <= hi; k += 256) bin_start[k] = val;
+    }
 }
 
 __global__ void __launch_bounds__(256)
@@ -149,20 +169,19 @@ int run_preorder(hcgrid_ctx* c, int64_t n, const double* lon, const double* lat,
     }
     if (c->opt_profile) cudaEventRecord(c->ev[2], st);
     {
+        // a4 (+ a5 in fp32 mode: the gather rides on the same pass over the sorted pairs)
         const unsigned nb2 = (unsigned)((nn + 1 + threads - 1) / threads);
-        bin_start_kernel<<<nb2, threads, 0, st>>>(c->d_keys_out.as<uint32_t>(), n, rg.nbins,
-                                                  c->d_bins.as<int32_t>());
+        tables_pack_kernel<<<nb2, threads, 0, st>>>(c->d_keys_out.as<uint32_t>(), c->d_idx_out.as<uint32_t>(), n,
+                                                    (int32_t)rg.nbins, c->d_bins.as<int32_t>(),
+                                                    f32 && n > 0 ? c->d_misc.as<Rec32>() : nullptr,
+                                                    c->d_rec.as<Rec32>());
         ++launches;
         HCG_CUDA(c, cudaGetLastError());
     }
     if (c->opt_profile) cudaEventRecord(c->ev[3], st);
-    if (n > 0) {
-        if (f32)
-            pack32_kernel<<<nb, threads, 0, st>>>(c->d_keys_out.as<uint32_t>(), c->d_idx_out.as<uint32_t>(), n,
-                                                  (uint32_t)rg.nbins, c->d_misc.as<Rec32>(), c->d_rec.as<Rec32>());
-        else
-            pack64_kernel<<<nb, threads, 0, st>>>(c->d_keys_out.as<uint32_t>(), c->d_idx_out.as<uint32_t>(), n,
-                                                  (uint32_t)rg.nbins, lon, lat, weights, c->d_rec.as<Rec64>());
+    if (n > 0 && !f32) {
+        pack64_kernel<<<nb, threads, 0, st>>>(c->d_keys_out.as<uint32_t>(), c->d_idx_out.as<uint32_t>(), n,
+                                              (uint32_t)rg.nbins, lon, lat, weights, c->d_rec.as<Rec64>());
         ++launches;
         HCG_CUDA(c, cudaGetLastError());
     }

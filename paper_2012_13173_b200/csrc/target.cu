@@ -150,6 +150,8 @@ static int finish_target(hcgrid_ctx* c, const std::vector<HostStrip>& hs, int st
     rg.lat_lo = kHalfPi - ring_colat(rl + 1, nside) - 1e-7;
     const double lat_hi = kHalfPi - ring_colat(rf - 1, nside) + 1e-7;
     rg.wy = lat_hi - rg.lat_lo;
+    rg.sx32 = 4294967296.0 / rg.wx;
+    rg.sy32 = 4294967296.0 / rg.wy;
     c->region = rg;
 
     // strips

@@ -136,6 +136,43 @@ def test_tile_shapes(oracle, cfg, shape):
     compare(cube2, wmap2, None, ref, w.sigma_deg, w.radius_deg, TOL_F32, qmax(w))
 
 
+@pytest.mark.parametrize("nchan", [4, 12, 64, 256, 300])
+def test_cube_kernel_channel_counts(oracle, nchan):
+    """conv_mc_f32 (stats kernel 7): partial lanes, exactly one and more than one 256-channel
+    block, weights, ragged 8 x 8 CTA tiles (the target is 23 x 19), with and without counts;
+    the general kernel on the same input as a second opinion."""
+    from paper_2012_13173_b200 import binding
+    rng = np.random.default_rng([5, nchan])
+    n = 5000
+    w = workloads.make(1, 1.0)
+    w.lon = 30.0 + rng.uniform(-0.3, 0.3, n)
+    w.lat = 20.0 + rng.uniform(-0.3, 0.3, n)
+    w.values = rng.normal(size=(n, nchan)).astype(np.float32)
+    w.weights = rng.uniform(0.5, 1.5, n).astype(np.float32)
+    w.target = workloads.CarTarget(23, 19, 29.8, 19.85, 1.0 / 60.0, 1.0 / 60.0)
+    ref = run_oracle(oracle, w)
+    cube, wmap, cnt, st = run_gpu(w, "f32")
+    assert st["kernel"] == 7
+    compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F32, qmax(w))
+    cube, wmap, cnt, st = run_gpu(w, "f32", want_counts=False)
+    compare(cube, wmap, None, ref, w.sigma_deg, w.radius_deg, TOL_F32, qmax(w))
+    cube, wmap, cnt, st = run_gpu(w, "f32", {binding.OPT_KERNEL: binding.KERNEL_GENERAL})
+    assert st["kernel"] == 3
+    compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F32, qmax(w))
+
+
+def test_cube_kernel_falls_back_for_odd_channel_counts(oracle):
+    w, ref = mini(oracle, 4)
+    w2 = workloads.make(4, MINI[4])
+    w2.values = np.ascontiguousarray(w2.values[:, :7])
+    ref2 = run_oracle(oracle, w2)
+    cube, wmap, cnt, st = run_gpu(w2, "f32")
+    assert st["kernel"] == 3
+    compare(cube, wmap, cnt, ref2, w2.sigma_deg, w2.radius_deg, TOL_F32)
+    _, _, _, st = run_gpu(w, "f32")
+    assert st["kernel"] == 7
+
+
 @pytest.mark.parametrize("radius_deg,sigma_deg", [(0.1, 0.04), (0.2, 0.08), (1.5, 0.5)])
 def test_tile_series_modes(oracle, radius_deg, sigma_deg):
     """Wider kernels switch the tile kernel's pair arithmetic to the series / full modes."""
@@ -151,6 +188,12 @@ def test_tile_series_modes(oracle, radius_deg, sigma_deg):
     cube, wmap, cnt, st = run_gpu(w, "f32")
     assert st["kernel"] == 6
     compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F32)
+    # the cube kernel shares the pair arithmetic: same modes with 8 channels
+    w.values = np.ascontiguousarray(np.repeat(w.values, 8, axis=1) * np.arange(1, 9, dtype=np.float32))
+    ref8 = run_oracle(oracle, w)
+    cube, wmap, cnt, st = run_gpu(w, "f32")
+    assert st["kernel"] == 7
+    compare(cube, wmap, cnt, ref8, w.sigma_deg, w.radius_deg, TOL_F32)
 
 
 @pytest.mark.parametrize("subpix", [0, 1, 3])
