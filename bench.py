@@ -34,6 +34,11 @@ if ROOT not in sys.path:
 
 METRIC = "gridded cell-channels/s (whole hcgrid_grid call, inputs resident in HBM)"
 UNIT = "cell-channels/s"
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` captures (profiles/): (config, stats kernel id) -> (bytes, source)
+NCU_TRAFFIC = {
+    (3, 6): (191923968 + 12062208, "profiles/r01b_conv1_tile_ncu_full.md"),
+}
 WORKLOAD_NAMES = {1: "config1_tiny_20k", 2: "config2_drift_scan_1.25M", 3: "config3_dense_10M",
                   4: "config4_spectral_cube_1M_x256", 5: "config5_polar_20M"}
 
@@ -159,10 +164,9 @@ def run_product(args):
     import torch
     import torch.distributed as dist
     from paper_2012_13173_b200 import binding, roofline, workloads
+    from paper_2012_13173_b200 import dist as hdist
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world, rank, local = hdist.env_world()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
     torch.cuda.set_device(local)
@@ -187,9 +191,7 @@ def run_product(args):
            torch.empty(ncell, dtype=torch.float32, device=dev), None)
 
     def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+        hdist.barrier(world, torch.cuda.synchronize)
 
     def step():
         g.grid(lon, lat, val, wts, want_counts=False, out=out)
@@ -255,10 +257,7 @@ def run_product(args):
     d2h = ncell * (4 * nchan + 4)
 
     # ---- max over ranks
-    if world > 1:
-        tmax = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device=dev)
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        ms_total, ms_e2e = float(tmax[0]), float(tmax[1])
+    ms_total, ms_e2e = hdist.max_over_ranks([ms_total, ms_e2e], world, dev)
     cnt = cnt_t.cpu().numpy().astype(np.int64)
     n_hit = int(cnt.sum())
     if rank != 0:
@@ -267,7 +266,7 @@ def run_product(args):
         return 0
 
     units = ncell * nchan * world
-    value = units * args.steps / (ms_total * 1e-3)
+    value = hdist.whole_job_rate(ncell * nchan, world, args.steps, ms_total)
     hbm_gbs, hbm_src = load_peaks()
     t_conv = float(np.mean(stage["us_convolve"])) * 1e-6
     cand = roofline.count_candidates(w, max_rows=args.cand_rows)
@@ -284,7 +283,10 @@ def run_product(args):
               "unit": "G FP32-pipe thread-inst/s"}
     rl["frac"] = rl["achieved"] / rl["peak"]
     rl.update({
-        "traffic": args.traffic,
+        "traffic": args.traffic if args.traffic is not None else (
+            NCU_TRAFFIC[(args.config, st["kernel"])][0]
+            if args.scale == 1.0 and (args.config, st["kernel"]) in NCU_TRAFFIC else None),
+        "traffic_source": NCU_TRAFFIC.get((args.config, st["kernel"]), (None, None))[1] if args.traffic is None else "--traffic",
         "kernel": {1: "conv1_simple_f32", 2: "conv1_staged_f32", 3: "conv_general<f32>", 4: "conv_general<f64 pair>",
                    5: "conv_general<f64>", 6: "conv1_tile_f32", 7: "conv_mc_f32"}.get(st["kernel"], str(st["kernel"])),
         "kernel_us": t_conv * 1e6, "t_roof_us": mdl["t_roof_s"] * 1e6,
