@@ -121,37 +121,30 @@ conv1_tile_f32(const TileArgs a) {
         __syncwarp();
         if (total == 0) continue;
 
-        // ---- steps (iv)+(v): the candidate stream, one record ahead in two named buffers.
-        // The trip count is warp-uniform; a lane past the end re-reads the last record and
-        // drops it by testing against a negative threshold.
+        // ---- steps (iv)+(v): the candidate stream, one record ahead.  Full steps (all 32 lanes
+        // inside the stream) need no validity test; the ragged last step tests against a negative
+        // threshold in the lanes past the end (they re-read the last record).
         const int last = total - 1;
-        const int niter = (total + 31) >> 5;
+        const int nfull = total >> 5;
         uint32_t tp = smem_addr(tab);                   // ring cursor: shared address of entry k
         unsigned long long end, base;
         lds_entry(tp, end, base);
         int i = lane;
         stream_seek(min(i, last), tp, end, base);
         uint4 ra = ldg_rec(base, min(i, last));
-        for (int it = 0; it < niter; it += 2) {
-            const int i1 = i + 32;
-            {
-                const int ii = min(i1, last);
-                stream_seek(ii, tp, end, base);
-                const uint4 rb = ldg_rec(base, ii);
-                tc.hm = i <= last ? tc.hmax : -1.0f;
-                tile_pairs<GX, GY, MODE, COUNTS>(ra, tc, W, S, cnt);
-                ra = rb;
-            }
-            if (it + 1 >= niter) break;
-            i += 64;
-            {
-                const int ii = min(i, last);
-                stream_seek(ii, tp, end, base);
-                const uint4 rb = ldg_rec(base, ii);
-                tc.hm = i1 <= last ? tc.hmax : -1.0f;
-                tile_pairs<GX, GY, MODE, COUNTS>(ra, tc, W, S, cnt);
-                ra = rb;
-            }
+        tc.hm = tc.hmax;
+#pragma unroll 2
+        for (int it = 0; it < nfull; ++it) {
+            i += 32;
+            const int ii = min(i, last);
+            stream_seek(ii, tp, end, base);
+            const uint4 rb = ldg_rec(base, ii);
+            tile_pairs<GX, GY, MODE, COUNTS>(ra, tc, W, S, cnt);
+            ra = rb;
+        }
+        if (total & 31) {
+            tc.hm = i <= last ? tc.hmax : -1.0f;
+            tile_pairs<GX, GY, MODE, COUNTS>(ra, tc, W, S, cnt);
         }
     }
 

@@ -362,9 +362,14 @@ def test_full_size_sampled_cells(oracle, cfg, k):
     w = workloads.make(cfg, 1.0)
     cells = sampled_cells(w.target.ncell, w.target.nx, k, cfg)
     ref = run_oracle(oracle, w, cells)
-    cube, wmap, cnt, st = run_gpu(w, "f32")          # default options = what bench.py times
+    cube, wmap, cnt, st = run_gpu(w, "f32")          # default options, with the count output
     r = compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F32, qmax(w), cells=cells)
     assert r["n_hit"] > 0
+    assert st["kernel"] == (7 if cfg == 4 else 6)
+    # exactly what bench.py times: default options, datacube + weight map only (no count output)
+    cube_b, wmap_b, none, st_b = run_gpu(w, "f32", want_counts=False)
+    assert none is None and st_b["kernel"] == st["kernel"]
+    compare(cube_b, wmap_b, None, ref, w.sigma_deg, w.radius_deg, TOL_F32, qmax(w), cells=cells)
     # properties that hold at any size: W > 0 <=> count > 0 <=> finite V; count bounded by n
     assert np.array_equal(wmap > 0, cnt > 0)
     assert np.array_equal(np.isfinite(cube[:, 0]), cnt > 0)
