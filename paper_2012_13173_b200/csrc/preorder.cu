@@ -13,7 +13,8 @@
 //                 table P_i -> S_start at bin granularity; its every m-th
 //                 entry is the second-level table R_start (Fig. 3).
 //   a5 pack       S -> S' ("rearrange the raw data S_n as S'") as 16-byte
-//                 fixed-point records (fp32 mode) or degree records (fp64 mode).
+//                 fixed-point records (fp32 mode) or degree records (fp64 mode).  In fp32
+//                 mode a4 and a5 are one kernel: one pass over the sorted pairs.
 #include <cub/device/device_radix_sort.cuh>
 
 #include "hcg_common.cuh"
