@@ -37,7 +37,8 @@ UNIT = "cell-channels/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` captures (profiles/): (config, stats kernel id) -> (bytes, source)
 NCU_TRAFFIC = {
-    (3, 6): (191923968 + 12062208, "profiles/r01b_conv1_tile_ncu_full.md"),
+    (3, 6): (191987968 + 11848960, "profiles/r01c_conv1_tile_ncu_full.md"),
+    (4, 7): (3888495000 + 99117824, "profiles/r01c_conv_mc_ncu_full.md"),
 }
 WORKLOAD_NAMES = {1: "config1_tiny_20k", 2: "config2_drift_scan_1.25M", 3: "config3_dense_10M",
                   4: "config4_spectral_cube_1M_x256", 5: "config5_polar_20M"}
