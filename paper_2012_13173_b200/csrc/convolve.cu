@@ -294,9 +294,9 @@ int run_convolve(hcgrid_ctx* c, int64_t n, const float* values, int nchan, bool 
     a.rg = rg; a.kp = c->kp;
     a.kmax = c->kmax; a.strip_cells = c->strip_cells;
     a.nchan = nchan;
-    a.qx = (float)(rg.wx / 4294967296.0);
-    a.qy = (float)(rg.wy / 4294967296.0);
-    a.sx = 4294967296.0 / rg.wx;
+    a.qx = (float)(1.0 / rg.sx32);
+    a.qy = (float)(1.0 / rg.sy32);
+    a.sx = rg.sx32;
     const bool f32 = c->precision == HCGRID_F32 && c->f32_series_ok && c->opt_kernel != 2;
     int rc;
     c->stats.coarsen_y = 1;
@@ -318,6 +318,7 @@ int run_convolve(hcgrid_ctx* c, int64_t n, const float* values, int nchan, bool 
         int G = c->opt_coarsen;
         if (G == 0) G = c->strip_cells >= 4 ? 2 : 1;
         if (G > c->strip_cells) G = 1;
+        if (rg.full_circle) G = 1;   // longitude differences are taken modulo the circle: one cell per task
         switch (G) {
             case 1: rc = launch_f32<1>(c, a, has_weights, staged, st); break;
             case 2: rc = launch_f32<2>(c, a, has_weights, staged, st); break;

@@ -219,8 +219,8 @@ void fill_tile_args(const hcgrid_ctx* c, int mode, TileArgs& a) {
     a.rec = c->d_rec.as<Rec32>();
     a.u0 = c->car_u0; a.du = c->car_du; a.sx = rg.sx32;
     a.nx = c->strip_cells; a.ny = c->nstrip; a.kmax = c->kmax; a.m = rg.m;
-    a.sxk = (float)(sk * rg.wx / 4294967296.0);
-    a.syk = (float)(sk * rg.wy / 4294967296.0);
+    a.sxk = (float)(sk / rg.sx32);
+    a.syk = (float)(sk / rg.sy32);
     a.duk = (float)(sk * c->car_du);
     a.dyk = (float)(sk * c->car_dlat);
     a.isk = (float)(1.0 / sk);

@@ -63,7 +63,7 @@ struct __align__(16) RowF {
 };
 
 // 16-byte packed sample S' as the fp32 convolution reads it (a5).  xi/yi are unsigned
-// fixed point over the region: lon offset u in [0, wx) -> xi = u / wx * 2^32 (wraps
+// fixed point over the region: lon offset u in [0, wx) -> xi = u * Region::sx32 (wraps
 // naturally when wx = 2 pi), lat offset -> yi.  Differences of two fixed-point
 // coordinates are exact integers, which is what keeps fp32 pair arithmetic at 1e-10 rad.
 struct __align__(16) Rec32 {
@@ -92,7 +92,7 @@ struct Region {            // what of the sphere the target can reach (host + de
     double lat_lo;         // rad
     double wy;             // rad, latitude extent mapped onto 2^32
     int64_t nbins;         // nring * m
-    double sx32, sy32;     // fixed-point units per radian: 2^32 / wx, 2^32 / wy
+    double sx32, sy32;     // fixed-point units per radian (lon, lat): 2^32 over a span >= wx / wy (target.cu)
 };
 
 struct KernelParams {      // per-context constants of the pair arithmetic

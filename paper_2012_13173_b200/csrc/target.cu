@@ -150,16 +150,26 @@ static int finish_target(hcgrid_ctx* c, const std::vector<HostStrip>& hs, int st
     rg.lat_lo = kHalfPi - ring_colat(rl + 1, nside) - 1e-7;
     const double lat_hi = kHalfPi - ring_colat(rf - 1, nside) + 1e-7;
     rg.wy = lat_hi - rg.lat_lo;
-    rg.sx32 = 4294967296.0 / rg.wx;
-    rg.sy32 = 4294967296.0 / rg.wy;
+    // Fixed-point scales of the packed records.  A kernel forms (int)(x_sample - x_cell0) for
+    // every candidate of a task, and a task's cell 0 can be up to 8 columns / rows away from the
+    // cell whose window brought the candidate in, so 2^32 must span at least twice that reach --
+    // otherwise the difference wraps (a target of a handful of cells is narrower than that).
+    {
+        const double du_abs = strip_cells > 1 ? std::fabs(hs[0].dlon_deg) * kDeg2Rad : 0.0;
+        const double dv_abs = strip_cells > 1 ? std::fabs(c->car_dlat) : 0.0;
+        const double ring_sp = (lat_hi - rg.lat_lo) / std::max(1, rg.nring);
+        const double span_x = rg.full_circle ? kTwoPi : std::max(rg.wx, 2.2 * (dlmax + 8.0 * du_abs));
+        const double span_y = std::max(rg.wy, 2.2 * (R + 8.0 * dv_abs + 3.0 * ring_sp));
+        rg.sx32 = 4294967296.0 / span_x;
+        rg.sy32 = 4294967296.0 / span_y;
+    }
     c->region = rg;
 
     // strips
     std::vector<Strip> st(hs.size());
     int kmax = 1;
     double cw = 1e9;
-    const double sx = 4294967296.0 / rg.wx, sy = 4294967296.0 / rg.wy;
-    (void)sx;
+    const double sy = rg.sy32;
     for (size_t i = 0; i < hs.size(); ++i) {
         Strip& s = st[i];
         const HostStrip& h = hs[i];
@@ -260,6 +270,7 @@ int build_target_cells(hcgrid_ctx* c, int64_t ncell, const double* lon, const do
     }
     c->is_car = false;
     c->ncell = ncell;
+    c->car_dlat = 0.0;
     return finish_target(c, hs, 1, lm + dmin, lm + dmax);
 }
 

@@ -378,3 +378,52 @@ def test_full_size_sampled_cells(oracle, cfg, k):
         # fp64 mode at the target config, same sampled cells
         cube, wmap, cnt, _ = run_gpu(w, "f64")
         compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F64, cells=cells)
+
+
+# ------------------------------------------------------------ randomised plate-carree targets
+def _random_car_case(seed):
+    """A seeded random problem: patch centre anywhere (including across lon = 0 and at high
+    latitude), random cell size / kernel width / nside / channel count / step signs."""
+    rng = np.random.default_rng([13173, 404, seed])
+    lat_c = float(rng.uniform(-84.0, 84.0))
+    lon_c = float(rng.choice([0.0, 359.7, 0.2, rng.uniform(0.0, 360.0)]))
+    sigma = float(rng.uniform(0.6, 3.0)) / 60.0
+    radius = sigma * float(rng.uniform(2.5, 4.0))
+    cell = sigma * float(rng.uniform(0.5, 1.2))
+    nx, ny = int(rng.integers(5, 42)), int(rng.integers(5, 34))
+    sx, sy = (1.0 if rng.random() < 0.5 else -1.0), (1.0 if rng.random() < 0.5 else -1.0)
+    dlon = sx * cell / max(np.cos(np.deg2rad(lat_c)), 0.05)      # roughly square cells on the sky
+    dlat = sy * cell
+    tgt = workloads.CarTarget(nx, ny, lon_c - 0.5 * (nx - 1) * dlon, lat_c - 0.5 * (ny - 1) * dlat, dlon, dlat)
+    half_lat = 0.5 * ny * cell + 1.5 * radius
+    half_lon = (0.5 * nx * cell + 1.5 * radius) / max(np.cos(np.deg2rad(lat_c)), 0.05)
+    n = int(rng.integers(2000, 9000))
+    lon = np.mod(lon_c + rng.uniform(-half_lon, half_lon, n), 360.0)
+    lat = np.clip(lat_c + rng.uniform(-half_lat, half_lat, n), -89.999, 89.999)
+    nchan = int(rng.choice([1, 1, 1, 8, 20]))
+    val = rng.standard_normal((n, nchan)).astype(np.float32)
+    wts = rng.uniform(0.5, 1.5, n).astype(np.float32) if rng.random() < 0.5 else None
+    nside = int(2 ** rng.integers(7, 14))
+    return tgt, lon, lat, val, wts, sigma, radius, nside
+
+
+@pytest.mark.parametrize("seed", range(16))
+def test_random_car_targets(oracle, seed):
+    """Default kernel choice (tile kernel for one channel, cube kernel for several) on random
+    plate-carree problems, fp32 and fp64 modes, against the oracle."""
+    from paper_2012_13173_b200 import binding
+    tgt, lon, lat, val, wts, sigma, radius, nside = _random_car_case(seed)
+    cl, cb = tgt.cell_centers()
+    ref = oracle.grid(sigma, radius, cl, cb, lon, lat, val, wts)
+    assert ref.counts.sum() > 0
+    for precision, tol in (("f32", TOL_F32), ("f64", TOL_F64)):
+        g = binding.HCGrid(sigma, radius, nside, precision=precision)
+        g.set_target_car(tgt.nx, tgt.ny, tgt.lon0, tgt.lat0, tgt.dlon, tgt.dlat)
+        cube, wmap, cnt = g.grid(_dev(lon), _dev(lat), _dev(val), None if wts is None else _dev(wts))
+        torch.cuda.synchronize()
+        st = g.stats()
+        if precision == "f32":
+            assert st["kernel"] in (6, 7, 3), st       # tile, cube, or the general kernel (nchan % 4 != 0)
+        compare(cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy(), ref, sigma, radius, tol,
+                1.5 if wts is not None else 1.0)
+        g.close()
