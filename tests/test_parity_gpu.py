@@ -407,7 +407,7 @@ def _random_car_case(seed):
     return tgt, lon, lat, val, wts, sigma, radius, nside
 
 
-@pytest.mark.parametrize("seed", range(16))
+@pytest.mark.parametrize("seed", range(48))
 def test_random_car_targets(oracle, seed):
     """Default kernel choice (tile kernel for one channel, cube kernel for several) on random
     plate-carree problems, fp32 and fp64 modes, against the oracle."""
@@ -427,3 +427,34 @@ def test_random_car_targets(oracle, seed):
         compare(cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy(), ref, sigma, radius, tol,
                 1.5 if wts is not None else 1.0)
         g.close()
+
+
+@pytest.mark.parametrize("nx,ny", [(1, 1), (2, 1), (1, 3), (3, 2), (5, 7), (9, 4), (4, 9)])
+def test_tiny_targets_every_tile_shape(oracle, nx, ny):
+    """Targets of a handful of cells: the region is barely wider than one support disc, tiles are
+    mostly ragged, and the farthest cell of a task is far from its cell 0 (the case that wrapped
+    the fixed-point differences before the span fix)."""
+    from paper_2012_13173_b200 import binding
+    rng = np.random.default_rng([13173, 505, nx, ny])
+    sigma, radius = 2.0 / 60.0, 6.5 / 60.0
+    n = 3000
+    lon = np.mod(359.9 + rng.uniform(-0.5, 0.5, n), 360.0)
+    lat = -47.0 + rng.uniform(-0.4, 0.4, n)
+    tgt = workloads.CarTarget(nx, ny, 359.9 + 0.03 * (nx - 1), -47.0 + 0.02 * (ny - 1), -0.06, -0.04)
+    cl, cb = tgt.cell_centers()
+    for nchan in (1, 4):
+        val = rng.standard_normal((n, nchan)).astype(np.float32)
+        ref = oracle.grid(sigma, radius, cl, cb, lon, lat, val, None)
+        assert ref.counts.min() > 0
+        shapes = TILE_SHAPES if nchan == 1 else [(0, 0)]
+        for shape in shapes:
+            g = binding.HCGrid(sigma, radius, 1024)
+            g.set_option(binding.OPT_COARSEN, shape[0])
+            g.set_option(binding.OPT_COARSEN_Y, shape[1])
+            g.set_target_car(tgt.nx, tgt.ny, tgt.lon0, tgt.lat0, tgt.dlon, tgt.dlat)
+            cube, wmap, cnt = g.grid(_dev(lon), _dev(lat), _dev(val))
+            torch.cuda.synchronize()
+            # a single-column target is a set of one-cell strips: it takes the staged / general kernels
+            assert g.stats()["kernel"] == ((6 if nchan == 1 else 7) if nx > 1 else (2 if nchan == 1 else 3))
+            compare(cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy(), ref, sigma, radius, TOL_F32)
+            g.close()
