@@ -458,3 +458,51 @@ def test_tiny_targets_every_tile_shape(oracle, nx, ny):
             assert g.stats()["kernel"] == ((6 if nchan == 1 else 7) if nx > 1 else (2 if nchan == 1 else 3))
             compare(cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy(), ref, sigma, radius, TOL_F32)
             g.close()
+
+
+@pytest.mark.parametrize("seed", range(24))
+def test_random_polar_and_wide_kernels(oracle, seed):
+    """Random plate-carree targets near the poles (whole-ring windows, full-circle regions) and
+    with wide kernels (series / full modes of the fp32 arithmetic, or the fp64 pair arithmetic when
+    the small-angle series is not valid), default kernel choice, fp32 mode."""
+    from paper_2012_13173_b200 import binding
+    rng = np.random.default_rng([13173, 606, seed])
+    polar = seed % 2 == 0
+    sign = 1.0 if rng.random() < 0.5 else -1.0
+    if polar:
+        lat_c = sign * float(rng.uniform(86.0, 89.3))
+        sigma = float(rng.uniform(2.0, 8.0)) / 60.0
+    else:
+        lat_c = float(rng.uniform(-70.0, 70.0))
+        sigma = float(rng.uniform(5.0, 40.0)) / 60.0          # up to 0.67 deg
+    radius = sigma * float(rng.uniform(2.5, 3.5))
+    cell = sigma * float(rng.uniform(0.6, 1.2))
+    nx, ny = int(rng.integers(4, 30)), int(rng.integers(3, 12))
+    ny = max(1, min(ny, int((89.95 - abs(lat_c)) / (0.5 * cell)))) if polar else ny
+    lon_c = float(rng.uniform(0.0, 360.0))
+    dlon = cell * float(rng.uniform(1.0, 6.0)) * (1.0 if rng.random() < 0.5 else -1.0)
+    dlat = cell * (1.0 if rng.random() < 0.5 else -1.0)
+    tgt = workloads.CarTarget(nx, ny, lon_c - 0.5 * (nx - 1) * dlon, lat_c - 0.5 * (ny - 1) * dlat, dlon, dlat)
+    cl, cb = tgt.cell_centers()
+    assert np.abs(cb).max() <= 90.0
+    n = 5000
+    half = 0.5 * ny * cell + 1.3 * radius
+    lat = np.clip(lat_c + rng.uniform(-half, half, n), -90.0, 90.0)
+    if polar:
+        lon = rng.uniform(0.0, 360.0, n)
+    else:
+        half_lon = 0.5 * nx * abs(dlon) + 1.3 * radius / np.cos(np.deg2rad(min(abs(lat_c) + half, 85.0)))
+        lon = np.mod(lon_c + rng.uniform(-half_lon, half_lon, n), 360.0)
+    nchan = int(rng.choice([1, 1, 4]))
+    val = rng.standard_normal((n, nchan)).astype(np.float32)
+    wts = rng.uniform(0.5, 1.5, n).astype(np.float32) if rng.random() < 0.5 else None
+    nside = int(2 ** rng.integers(5, 11))
+    ref = oracle.grid(sigma, radius, cl, cb, lon, lat, val, wts)
+    assert ref.counts.sum() > 0
+    g = binding.HCGrid(sigma, radius, nside)
+    g.set_target_car(tgt.nx, tgt.ny, tgt.lon0, tgt.lat0, tgt.dlon, tgt.dlat)
+    cube, wmap, cnt = g.grid(_dev(lon), _dev(lat), _dev(val), None if wts is None else _dev(wts))
+    torch.cuda.synchronize()
+    compare(cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy(), ref, sigma, radius, TOL_F32,
+            1.5 if wts is not None else 1.0)
+    g.close()
