@@ -11,7 +11,7 @@
 //   phase 1 (per 32 candidates): lane = candidate; the 8 kernel weights of the sub-tile by
 //           the tile kernel's scaled fp32 pair arithmetic; weight map / counts accumulated
 //           per lane; candidates that hit at least one of the 8 cells are compacted into a
-//           per-warp shared-memory list (weights stored as duplicated pairs + sample index)
+//           per-warp shared-memory list (8 weights + the row's address)
 //   phase 2 (per listed candidate): the warp copies the sample's spectrum row in place
 //           (values are never moved: a5) into a 4-deep shared-memory ring with cp.async,
 //           three rows ahead of the arithmetic, and does 8 cells x 8 channels of FMAs as
@@ -33,7 +33,7 @@ struct McArgs {
 constexpr int kMcWarps = 8;
 constexpr int kMcTile = 8;         // CTA tile edge in cells
 constexpr int kSX = 4, kSY = 2;    // sub-tile of one warp
-constexpr int kHitStride = 20;     // floats per list entry: 8 duplicated weights + index + pad (80 B)
+constexpr int kHitStride = 12;     // floats per list entry: 8 weights + row address + pad (48 B)
 constexpr int kRowDepth = 4;       // spectrum rows in flight per warp (cp.async ring)
 constexpr int kMcSmemWarp = 32 * 16 + 32 * kHitStride * 4 + kRowDepth * 1024 + 2 * 1024;   // table + list + rows + W + counts
 
@@ -237,11 +237,9 @@ conv_mc_f32(const McArgs m) {
                 const unsigned mask = __ballot_sync(0xffffffffu, hits != 0);
                 if (hits != 0) {
                     float* e = hitl + __popc(mask & ((1u << lane) - 1u)) * kHitStride;
-                    *(float4*)(e + 0) = make_float4(wq[0], wq[0], wq[1], wq[1]);
-                    *(float4*)(e + 4) = make_float4(wq[2], wq[2], wq[3], wq[3]);
-                    *(float4*)(e + 8) = make_float4(wq[4], wq[4], wq[5], wq[5]);
-                    *(float4*)(e + 12) = make_float4(wq[6], wq[6], wq[7], wq[7]);
-                    *(unsigned long long*)(e + 16) =
+                    *(float4*)(e + 0) = make_float4(wq[0], wq[1], wq[2], wq[3]);
+                    *(float4*)(e + 4) = make_float4(wq[4], wq[5], wq[6], wq[7]);
+                    *(unsigned long long*)(e + 8) =
                         (unsigned long long)(uintptr_t)(m.values + (size_t)cur.z * nchan + ch0);
                     float4 w0 = *(float4*)wacc, w1 = *(float4*)(wacc + 4);
                     w0.x += wq[0]; w0.y += wq[1]; w0.z += wq[2]; w0.w += wq[3];
@@ -261,7 +259,7 @@ conv_mc_f32(const McArgs m) {
                 if (nhit > 0) {
                     auto issue = [&](uint32_t ent_s, uint32_t dst) {
                         unsigned long long rp;
-                        asm volatile("ld.shared.u64 %0, [%1+64];" : "=l"(rp) : "r"(ent_s));
+                        asm volatile("ld.shared.u64 %0, [%1+32];" : "=l"(rp) : "r"(ent_s));
                         rp += chl_bytes;
                         if (ok0) cp_async16(dst, (const void*)(uintptr_t)rp);
                         if (ok1) cp_async16(dst + 16, (const void*)(uintptr_t)(rp + 16));
@@ -284,18 +282,17 @@ conv_mc_f32(const McArgs m) {
                         const float4 va = lds128(src), vb = lds128(src + 16);
                         const unsigned long long v01 = pack2(va.x, va.y), v23 = pack2(va.z, va.w);
                         const unsigned long long v45 = pack2(vb.x, vb.y), v67 = pack2(vb.z, vb.w);
+                        // the 8 weights by two broadcast loads; each is paired with itself in registers
+                        // (duplicated pairs in shared memory cost twice the load/store-pipe cycles)
+                        const float4 wlo = lds128(ent_s), whi = lds128(ent_s + 16);
+                        const float wv[8] = {wlo.x, wlo.y, wlo.z, wlo.w, whi.x, whi.y, whi.z, whi.w};
 #pragma unroll
-                        for (int c4 = 0; c4 < 4; ++c4) {
-                            unsigned long long wa, wb;          // (w,w) of cells 2c4, 2c4+1
-                            asm volatile("ld.shared.v2.u64 {%0, %1}, [%2];" : "=l"(wa), "=l"(wb) : "r"(ent_s + 16 * c4));
-                            acc[2 * c4][0] = ffma2(v01, wa, acc[2 * c4][0]);
-                            acc[2 * c4][1] = ffma2(v23, wa, acc[2 * c4][1]);
-                            acc[2 * c4][2] = ffma2(v45, wa, acc[2 * c4][2]);
-                            acc[2 * c4][3] = ffma2(v67, wa, acc[2 * c4][3]);
-                            acc[2 * c4 + 1][0] = ffma2(v01, wb, acc[2 * c4 + 1][0]);
-                            acc[2 * c4 + 1][1] = ffma2(v23, wb, acc[2 * c4 + 1][1]);
-                            acc[2 * c4 + 1][2] = ffma2(v45, wb, acc[2 * c4 + 1][2]);
-                            acc[2 * c4 + 1][3] = ffma2(v67, wb, acc[2 * c4 + 1][3]);
+                        for (int c = 0; c < 8; ++c) {
+                            const unsigned long long ww = pack2(wv[c], wv[c]);
+                            acc[c][0] = ffma2(v01, ww, acc[c][0]);
+                            acc[c][1] = ffma2(v23, ww, acc[c][1]);
+                            acc[c][2] = ffma2(v45, ww, acc[c][2]);
+                            acc[c][3] = ffma2(v67, ww, acc[c][3]);
                         }
                     }
                 }
