@@ -34,11 +34,11 @@ constexpr int kMcWarps = 8;
 constexpr int kMcTile = 8;         // CTA tile edge in cells
 constexpr int kSX = 4, kSY = 2;    // sub-tile of one warp
 constexpr int kHitStride = 12;     // floats per list entry: 8 weights + row address + pad (48 B)
-constexpr int kRowDepth = 4;       // spectrum rows in flight per warp (cp.async ring)
+constexpr int kRowDepth = 8;       // spectrum rows in flight per warp (cp.async ring)
 constexpr int kMcSmemWarp = 32 * 16 + 32 * kHitStride * 4 + kRowDepth * 1024 + 2 * 1024;   // table + list + rows + W + counts
 
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
