@@ -38,7 +38,7 @@ UNIT = "cell-channels/s"
 # `ncu --set full` captures (profiles/): (config, stats kernel id) -> (bytes, source)
 NCU_TRAFFIC = {
     (3, 6): (191987968 + 11848960, "profiles/r01c_conv1_tile_ncu_full.md"),
-    (4, 7): (3888495000 + 99117824, "profiles/r01c_conv_mc_ncu_full.md"),
+    (4, 7): (3714980000 + 98979072, "profiles/r01c_conv_mc_ncu_full.md"),
 }
 WORKLOAD_NAMES = {1: "config1_tiny_20k", 2: "config2_drift_scan_1.25M", 3: "config3_dense_10M",
                   4: "config4_spectral_cube_1M_x256", 5: "config5_polar_20M"}

@@ -5,20 +5,20 @@
 //
 // A CTA of 8 warps owns 8 x 8 target cells; warp w owns the 4 x 2 sub-tile (w & 1, w >> 1) and
 // all channels of a 256-channel block, lane l holding channels 8l .. 8l+7 of its 8 cells in
-// 64 accumulators (32 register pairs).  All warps of the CTA walk the SAME candidate stream
-// (the union window of the 8 x 8 cells, built as in convolve_tile.cu) in the same order, so
-// a sample's spectrum row is pulled from L2 once per CTA and then served by L1.
+// 64 accumulators (32 register pairs).  Every warp walks the candidate stream of its own
+// sub-tile (built as in convolve_tile.cu); the 8 warps of a CTA are neighbours on the sky,
+// so the spectrum rows they share are found in L2.
 //   phase 1 (per 32 candidates): lane = candidate; the 8 kernel weights of the sub-tile by
 //           the tile kernel's scaled fp32 pair arithmetic; weight map / counts accumulated
 //           per lane; candidates that hit at least one of the 8 cells are compacted into a
 //           per-warp shared-memory list (8 weights + the row's address)
 //   phase 2 (per listed candidate): the warp copies the sample's spectrum row in place
-//           (values are never moved: a5) into a 4-deep shared-memory ring with cp.async,
-//           three rows ahead of the arithmetic, and does 8 cells x 8 channels of FMAs as
-//           32 packed fma.rn.f32x2, so the FP32 pipe, not the issue slot, bounds it.
-// CTA rows alternate the ring direction of the stream (north to south, then south to north),
-// so vertically adjacent CTAs, which start together, meet their shared samples at the same
-// time and the spectra are fetched from HBM about once instead of once per CTA row.
+//           (values are never moved: a5) into an 8-deep shared-memory ring with cp.async.cg
+//           (L2 only: going through L1 cost 30 %), seven rows ahead of the arithmetic, and
+//           does 8 cells x 8 channels of FMAs as 32 packed fma.rn.f32x2.
+// Sub-tile rows alternate the ring direction of the stream (north to south, then south to
+// north), so vertically adjacent sub-tiles, which start together, meet their shared samples
+// at about the same time.
 // Reductions in a fixed order, no atomics.
 #include "hcg_tile.cuh"
 
@@ -110,8 +110,6 @@ conv_mc_f32(const McArgs m) {
     const int cty = (int)(blockIdx.x / (unsigned)a.tiles_x);
     const int cix0 = (int)(blockIdx.x - (unsigned)cty * (unsigned)a.tiles_x) * kMcTile;
     const int crow0 = cty * kMcTile;
-    const int ccols = min(kMcTile, a.nx - cix0);
-    const int crows = min(kMcTile, a.ny - crow0);
     const int ix0 = cix0 + kSX * (wib & 1);
     const int row0 = crow0 + kSY * (wib >> 1);
     const int ncols = min(kSX, a.nx - ix0);
@@ -140,15 +138,15 @@ conv_mc_f32(const McArgs m) {
     tc.sxk = a.sxk; tc.syk = a.syk; tc.duk = a.duk; tc.dyk = a.dyk;
     tc.a12 = a.a12; tc.hmax = a.hmax; tc.hm = a.hmax;
 
-    // ---- ring range of the CTA tile (every warp of the CTA computes the same stream)
+    // ---- ring range of the sub-tile
     int rmin = 0x7fffffff, rmax = -0x7fffffff;
-    for (int j = 0; j < crows; ++j) {
-        const int4 r0 = __ldg((const int4*)(a.rows + crow0 + j));
+    for (int j = 0; j < nrows; ++j) {
+        const int4 r0 = __ldg((const int4*)(a.rows + row0 + j));
         rmin = min(rmin, r0.y);
         rmax = max(rmax, r0.y + r0.z - 1);
     }
-    const float fxw = (float)(a.du >= 0.0 ? cix0 : cix0 + ccols - 1);
-    const float fxe = (float)(a.du >= 0.0 ? cix0 + ccols - 1 : cix0);
+    const float fxw = (float)(a.du >= 0.0 ? ix0 : ix0 + ncols - 1);
+    const float fxe = (float)(a.du >= 0.0 ? ix0 + ncols - 1 : ix0);
     const Rec32* __restrict__ rec = a.rec;
     unsigned char* wsm = s_mc + (size_t)wib * kMcSmemWarp;
     ulonglong2* tab = (ulonglong2*)wsm;
@@ -159,7 +157,7 @@ conv_mc_f32(const McArgs m) {
     float* wacc = (float*)(wsm + 32 * 16 + 32 * kHitStride * 4 + kRowDepth * 1024) + lane * 8;
     int* cacc = (int*)(wacc + 256 - lane * 8) + lane * 8;
     const int nchan = m.nchan;
-    const bool flip = (cty & 1) != 0;                       // odd CTA rows walk the rings south to north
+    const bool flip = ((row0 / kSY) & 1) != 0;              // odd sub-tile rows walk the rings south to north
 
     for (int ch0 = 0; ch0 < nchan; ch0 += 256) {
         const int chl = ch0 + 8 * lane;                      // first channel of this lane
@@ -176,14 +174,14 @@ conv_mc_f32(const McArgs m) {
         const unsigned long long chl_bytes = (unsigned long long)(32 * lane);   // this lane's 8 channels of the block
 
         for (int rb = 0; rb <= rmax - rmin; rb += 32) {
-            // ---- steps (ii)+(iii) for the CTA tile: lane k <-> ring number k of this pass
+            // ---- steps (ii)+(iii) for the sub-tile: lane k <-> ring number k of this pass
             const int r = flip ? rmax - rb - lane : rmin + rb + lane;
             int jlo = 0x7fffffff, jhi = -1;
-            for (int j = 0; j < crows; ++j) {
-                const int4 r0 = __ldg((const int4*)(a.rows + crow0 + j));
+            for (int j = 0; j < nrows; ++j) {
+                const int4 r0 = __ldg((const int4*)(a.rows + row0 + j));
                 const int k = r - r0.y;
                 if (k >= 0 && k < r0.z) {
-                    const float4 w = __ldg((const float4*)(a.wins + (size_t)(crow0 + j) * a.kmax + k));
+                    const float4 w = __ldg((const float4*)(a.wins + (size_t)(row0 + j) * a.kmax + k));
                     const int fl = __float_as_int(w.w);
                     if (fl == 1) {
                         jlo = min(jlo, __float2int_rd(fmaf(fxw, w.z, w.x)));
