@@ -506,3 +506,31 @@ def test_random_polar_and_wide_kernels(oracle, seed):
     compare(cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy(), ref, sigma, radius, TOL_F32,
             1.5 if wts is not None else 1.0)
     g.close()
+
+
+def test_large_sparse_target(oracle):
+    """A 2048 x 2048 target (4.2 M cells) of which only a corner holds samples: every tile far from
+    the data is empty (NaN / 0 / 0), the cells near the data match the oracle."""
+    from paper_2012_13173_b200 import binding
+    rng = np.random.default_rng([13173, 707])
+    n = 40000
+    tgt = workloads.CarTarget(2048, 2048, 100.0, -8.0, 0.5 / 60.0, 0.5 / 60.0)
+    lon = 100.0 + rng.uniform(0.0, 0.4, n)
+    lat = -8.0 + rng.uniform(0.0, 0.3, n)
+    val = rng.standard_normal((n, 1)).astype(np.float32)
+    sigma, radius = 0.5 / 60.0, 1.5 / 60.0
+    g = binding.HCGrid(sigma, radius, 4096)
+    g.set_target_car(tgt.nx, tgt.ny, tgt.lon0, tgt.lat0, tgt.dlon, tgt.dlat)
+    cube, wmap, cnt = g.grid(_dev(lon), _dev(lat), _dev(val))
+    torch.cuda.synchronize()
+    assert g.stats()["kernel"] == 6
+    cube, wmap, cnt = cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy()
+    g.close()
+    iy, ix = np.divmod(np.arange(tgt.ncell), tgt.nx)
+    far = (ix > 60) | (iy > 48)                      # beyond the data + support radius
+    assert (cnt[far] == 0).all() and (wmap[far] == 0).all() and np.isnan(cube[far, 0]).all()
+    assert int(cnt.sum()) > 0
+    cells = np.flatnonzero(~far)[::7]
+    cl, cb = tgt.cell_centers()
+    ref = oracle.grid(sigma, radius, cl[cells], cb[cells], lon, lat, val, None)
+    compare(cube, wmap, cnt, ref, sigma, radius, TOL_F32, cells=cells)
