@@ -67,7 +67,8 @@ enum {
                                     5 = force the tile kernel (error if the target does not allow it);
                                     6 = force the cube kernel (nchan > 1; error if not applicable) */
     HCGRID_OPT_WARPS_PER_SM = 5, /* resident convolution warps per SM (staged kernel); 0 = auto */
-    HCGRID_OPT_COARSEN_Y = 6     /* target rows per warp task (tile kernel); 0 = auto */
+    HCGRID_OPT_COARSEN_Y = 6,    /* target rows per warp task (tile kernel); 0 = auto */
+    HCGRID_OPT_SPLIT = 7         /* warps sharing one tile's candidate stream (tile kernel): 1, 2, 4; 0 = auto */
 };
 
 typedef struct {
@@ -81,6 +82,8 @@ typedef struct {
     int32_t gpu_launches;     /* kernels launched by the last hcgrid_grid                     */
     int32_t coarsen_y;        /* target rows per warp task used (tile kernel; else 1)         */
     float us_pixelise, us_sort, us_tables, us_pack, us_convolve, us_total; /* PROFILE only   */
+    int32_t split;            /* warps per tile used (tile kernel; else 1)                    */
+    int32_t reserved;
 } hcgrid_stats;
 
 /* Create a context.  sigma_deg = kernel standard deviation, support_radius_deg =

@@ -116,6 +116,11 @@ int hcgrid_set_option(hcgrid_ctx* c, int option, int64_t value) {
             if (value < 0 || value > 64) return fail(c, HCGRID_ERR_INVALID_ARG, "warps per SM must be 0..64");
             c->opt_warps = (int)value;
             break;
+        case HCGRID_OPT_SPLIT:
+            if (value != 0 && value != 1 && value != 2 && value != 4)
+                return fail(c, HCGRID_ERR_INVALID_ARG, "split must be 0 (auto), 1, 2 or 4");
+            c->opt_split = (int)value;
+            break;
         default: return fail(c, HCGRID_ERR_INVALID_ARG, "unknown option %d", option);
     }
     return HCGRID_OK;

@@ -300,6 +300,7 @@ int run_convolve(hcgrid_ctx* c, int64_t n, const float* values, int nchan, bool 
     const bool f32 = c->precision == HCGRID_F32 && c->f32_series_ok && c->opt_kernel != 2;
     int rc;
     c->stats.coarsen_y = 1;
+    c->stats.split = 1;
     if (c->opt_kernel == 5 && !(f32 && nchan == 1 && c->tile_ok))
         return fail(c, HCGRID_ERR_UNSUPPORTED, "the tile kernel needs fp32 mode, one channel and a plate-carree "
                     "target whose reach is a plain longitude window");

@@ -24,17 +24,25 @@
 
 namespace hcg {
 
-constexpr int kTileWarps = 4;
+constexpr int kTileWarps = 4;        // warps (= tiles) per CTA when tiles are not split
+constexpr int kMaxTileWarps = 4;     // largest split: warps of one CTA on one tile
 
-template <int GX, int GY, int MODE, bool COUNTS>
-__global__ void __launch_bounds__(kTileWarps * 32)
+template <int GX, int GY, int MODE, bool COUNTS, bool SPLIT>
+__global__ void __launch_bounds__(kMaxTileWarps * 32)
 conv1_tile_f32(const TileArgs a) {
     constexpr int NC = GX * GY;
-    __shared__ ulonglong2 s_tab[kTileWarps][32];
+    __shared__ ulonglong2 s_tab[kMaxTileWarps][32];
+    __shared__ float s_pw[SPLIT ? kMaxTileWarps : 1][NC], s_ps[SPLIT ? kMaxTileWarps : 1][NC];   // partial sums of a split tile
+    __shared__ int s_pc[SPLIT ? kMaxTileWarps : 1][NC];
     const int lane = threadIdx.x & 31;
     const int wib = threadIdx.x >> 5;
-    const unsigned tile = blockIdx.x * kTileWarps + wib;         // ntiles <= 2^30 (api.cu)
-    if (tile >= (unsigned)a.ntiles) return;
+    // a.split == 1: the CTA's warps own consecutive tiles.  a.split == S > 1 (few tiles, long streams):
+    // the CTA is S warps on ONE tile, warp p taking the stream steps p, p + S, ...; their partial sums
+    // are added in warp order through shared memory (fixed order, no atomics).
+    const int S = SPLIT ? a.split : 1;                          // SPLIT = false compiles to the plain one-warp-per-tile kernel
+    const int part = SPLIT ? wib : 0;
+    const unsigned tile = SPLIT ? blockIdx.x : blockIdx.x * kTileWarps + wib;   // ntiles <= 2^30 (api.cu)
+    if (tile >= (unsigned)a.ntiles) return;                     // the whole CTA when S > 1
     const int ty = (int)(tile / (unsigned)a.tiles_x);
     const int ix0 = (int)(tile - (unsigned)ty * (unsigned)a.tiles_x) * GX;
     const int row0 = ty * GY;
@@ -71,10 +79,10 @@ conv1_tile_f32(const TileArgs a) {
     tc.sxk = a.sxk; tc.syk = a.syk; tc.duk = a.duk; tc.dyk = a.dyk;
     tc.a12 = a.a12; tc.hmax = a.hmax;
 
-    float W[NC], S[NC];
+    float W[NC], S_[NC];
     int cnt[NC];
 #pragma unroll
-    for (int c = 0; c < NC; ++c) { W[c] = 0.f; S[c] = 0.f; cnt[c] = 0; }
+    for (int c = 0; c < NC; ++c) { W[c] = 0.f; S_[c] = 0.f; cnt[c] = 0; }
 
     const float fxw = (float)(a.du >= 0.0 ? ix0 : ix0 + ncols - 1);   // westmost / eastmost column of the tile
     const float fxe = (float)(a.du >= 0.0 ? ix0 + ncols - 1 : ix0);
@@ -126,42 +134,54 @@ conv1_tile_f32(const TileArgs a) {
         // threshold in the lanes past the end (they re-read the last record).
         const int last = total - 1;
         const int nfull = total >> 5;
+        const int stride = 32 * S;
         uint32_t tp = smem_addr(tab);                   // ring cursor: shared address of entry k
         unsigned long long end, base;
         lds_entry(tp, end, base);
-        int i = lane;
+        int i = part * 32 + lane;
         stream_seek(min(i, last), tp, end, base);
         uint4 ra = ldg_rec(base, min(i, last));
         tc.hm = tc.hmax;
 #pragma unroll 2
-        for (int it = 0; it < nfull; ++it) {
-            i += 32;
+        for (int it = part; it < nfull; it += S) {
+            i += stride;
             const int ii = min(i, last);
             stream_seek(ii, tp, end, base);
             const uint4 rb = ldg_rec(base, ii);
-            tile_pairs<GX, GY, MODE, COUNTS>(ra, tc, W, S, cnt);
+            tile_pairs<GX, GY, MODE, COUNTS>(ra, tc, W, S_, cnt);
             ra = rb;
         }
-        if (total & 31) {
+        if ((total & 31) && (nfull & (S - 1)) == part) {  // the ragged last step belongs to one warp
             tc.hm = i <= last ? tc.hmax : -1.0f;
-            tile_pairs<GX, GY, MODE, COUNTS>(ra, tc, W, S, cnt);
+            tile_pairs<GX, GY, MODE, COUNTS>(ra, tc, W, S_, cnt);
         }
     }
 
-    // ---- finish: transposed reduction, normalise, store
+    // ---- finish: transposed reduction, (split tiles: partial sums through shared memory), normalise, store
     TileReduce<NC, 16, float>::run(W, lane);
-    TileReduce<NC, 16, float>::run(S, lane);
+    TileReduce<NC, 16, float>::run(S_, lane);
     if (COUNTS) TileReduce<NC, 16, int>::run(cnt, lane);
     constexpr int SHIFT = 5 - ilog2(NC);
-    if ((lane & ((1 << SHIFT) - 1)) == 0) {
-        const int c = lane >> SHIFT;
+    const bool writer = (lane & ((1 << SHIFT) - 1)) == 0;
+    const int c = lane >> SHIFT;
+    float wsum = W[0], ssum = S_[0];
+    int csum = cnt[0];
+    if (SPLIT) {
+        if (writer) { s_pw[wib][c] = wsum; s_ps[wib][c] = ssum; s_pc[wib][c] = csum; }
+        __syncthreads();
+        if (wib != 0) return;
+        if (writer) {
+            wsum = s_pw[0][c]; ssum = s_ps[0][c]; csum = s_pc[0][c];
+            for (int w = 1; w < S; ++w) { wsum += s_pw[w][c]; ssum += s_ps[w][c]; csum += s_pc[w][c]; }
+        }
+    }
+    if (writer) {
         const int gx = c % GX, gy = c / GX;
         if (gx < ncols && gy < nrows) {
             const int64_t cell = (int64_t)(row0 + gy) * a.nx + ix0 + gx;
-            const float w = W[0];
-            a.cube[cell] = w > 0.0f ? S[0] / w : __int_as_float(0x7fc00000);
-            a.wmap[cell] = w;
-            if (COUNTS) a.counts[cell] = cnt[0];
+            a.cube[cell] = wsum > 0.0f ? ssum / wsum : __int_as_float(0x7fc00000);
+            a.wmap[cell] = wsum;
+            if (COUNTS) a.counts[cell] = csum;
         }
     }
 }
@@ -169,9 +189,13 @@ conv1_tile_f32(const TileArgs a) {
 // ------------------------------------------------------------------ launcher
 template <int GX, int GY>
 static cudaError_t launch_shape(const TileArgs& a, int mode, bool counts, cudaStream_t st) {
-    const unsigned blocks = (unsigned)((a.ntiles + kTileWarps - 1) / kTileWarps);
-    const int threads = kTileWarps * 32;
-#define HCG_TILE(M, C) conv1_tile_f32<GX, GY, M, C><<<blocks, threads, 0, st>>>(a)
+    const unsigned blocks = a.split > 1 ? (unsigned)a.ntiles : (unsigned)((a.ntiles + kTileWarps - 1) / kTileWarps);
+    const int threads = (a.split > 1 ? a.split : kTileWarps) * 32;
+#define HCG_TILE(M, C)                                                                 \
+    do {                                                                               \
+        if (a.split > 1) conv1_tile_f32<GX, GY, M, C, true><<<blocks, threads, 0, st>>>(a);  \
+        else conv1_tile_f32<GX, GY, M, C, false><<<blocks, threads, 0, st>>>(a);       \
+    } while (0)
     switch (mode * 2 + (counts ? 1 : 0)) {
         case 0: HCG_TILE(0, false); break;
         case 1: HCG_TILE(0, true); break;
@@ -226,6 +250,7 @@ void fill_tile_args(const hcgrid_ctx* c, int mode, TileArgs& a) {
     a.isk = (float)(1.0 / sk);
     a.a12 = (float)(1.0 / (12.0 * kappa));
     a.hmax = (float)(mode == 0 ? kappa * kp.radius * kp.radius : kappa * 4.0 * kp.hav_max);
+    a.split = 1;
 }
 
 int launch_conv_tile(hcgrid_ctx* c, int64_t n, float* cube, float* wmap, int32_t* counts, cudaStream_t st) {
@@ -262,6 +287,22 @@ int launch_conv_tile(hcgrid_ctx* c, int64_t n, float* cube, float* wmap, int32_t
     a.cube = cube; a.wmap = wmap; a.counts = counts;
     a.tiles_x = (nx + gx - 1) / gx;
     a.ntiles = (int64_t)a.tiles_x * ((ny + gy - 1) / gy);
+    // Few tiles with long candidate streams (the paper's own experiments: 90 x 90 cells, up to
+    // 3.6e8 samples) cannot fill 148 SMs with one warp per tile: split every
+    // tile's stream over S warps of one CTA until about 48 warps per SM exist, as long as each
+    // warp keeps at least 8 stream steps.
+    int split = c->opt_split;
+    if (split == 0) {
+        split = 1;
+        const double two_r = 2.0 * kp.radius;
+        const double ring_sp = rg.wy / std::max(1, rg.nring);
+        const double dens = (double)n / std::max(1e-300, rg.wx * rg.wy);
+        const double steps = dens * (2.0 * c->dlmax + (gx - 1) * std::fabs(c->car_du)) *
+                             (two_r + 2.0 * ring_sp + (gy - 1) * std::fabs(c->car_dlat)) / 32.0;
+        const double want = 48.0 * c->num_sms;
+        while (split < kMaxTileWarps && (double)a.ntiles * split < want && steps / (2 * split) >= 8.0) split *= 2;
+    }
+    a.split = split;
 
     cudaError_t e = cudaSuccess;
     bool built = false;
@@ -274,6 +315,7 @@ int launch_conv_tile(hcgrid_ctx* c, int64_t n, float* cube, float* wmap, int32_t
     if (e != cudaSuccess) return cuda_fail(c, e, "conv1_tile_f32");
     c->stats.coarsen = gx;
     c->stats.coarsen_y = gy;
+    c->stats.split = split;
     return HCGRID_OK;
 }
 

@@ -534,3 +534,37 @@ def test_large_sparse_target(oracle):
     cl, cb = tgt.cell_centers()
     ref = oracle.grid(sigma, radius, cl[cells], cb[cells], lon, lat, val, None)
     compare(cube, wmap, cnt, ref, sigma, radius, TOL_F32, cells=cells)
+
+
+@pytest.mark.parametrize("split", [1, 2, 4])
+@pytest.mark.parametrize("shape", [(1, 1), (4, 2), (8, 2)], ids=lambda s: f"{s[0]}x{s[1]}")
+def test_split_tiles(oracle, shape, split):
+    """Tile kernel with every tile's candidate stream shared by `split` warps of one CTA (few
+    cells, many samples per cell: the paper's 90 x 90-cell experiments), forced and automatic."""
+    from paper_2012_13173_b200 import binding
+    rng = np.random.default_rng([13173, 808])
+    n = 60000
+    sigma, radius = 127.4 / 3600.0, 382.2 / 3600.0
+    lon = 30.0 + rng.uniform(-0.6, 0.6, n)
+    lat = 25.0 + rng.uniform(-0.6, 0.6, n)
+    val = rng.standard_normal((n, 1)).astype(np.float32)
+    wts = rng.uniform(0.5, 1.5, n).astype(np.float32)
+    tgt = workloads.CarTarget(13, 11, 29.7, 24.75, 200.0 / 3600.0, 200.0 / 3600.0)
+    cl, cb = tgt.cell_centers()
+    ref = oracle.grid(sigma, radius, cl, cb, lon, lat, val, wts)
+    opts = {binding.OPT_KERNEL: binding.KERNEL_TILE, binding.OPT_COARSEN: shape[0], binding.OPT_COARSEN_Y: shape[1],
+            binding.OPT_SPLIT: split}
+    for counts in (True, False):
+        cube, wmap, cnt, st = run_gpu(wl_like(tgt, lon, lat, val, wts, sigma, radius), "f32", opts, want_counts=counts)
+        assert st["split"] == split
+        compare(cube, wmap, cnt, ref, sigma, radius, TOL_F32, 1.5)
+    if shape == (4, 2) and split == 1:
+        _, _, _, st = run_gpu(wl_like(tgt, lon, lat, val, wts, sigma, radius), "f32")
+        assert st["split"] > 1          # 143 cells x ~5,000 contributors each: the automatic choice splits
+
+
+def wl_like(tgt, lon, lat, val, wts, sigma, radius, nside=2048):
+    w = workloads.make(1, 1.0)
+    w.lon, w.lat, w.values, w.weights, w.target = lon, lat, val, wts, tgt
+    w.sigma_deg, w.radius_deg, w.nside = sigma, radius, nside
+    return w
