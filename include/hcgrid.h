@@ -121,6 +121,23 @@ int hcgrid_grid_host(hcgrid_ctx* ctx, int64_t n, const double* lon_deg, const do
                      const float* values, int32_t nchan, const float* weights,
                      void* datacube, void* weightmap, int32_t* counts);
 
+/* Incremental gridding: successive batches of samples (successive scans) into one cube.
+ * Eq. 1 is a ratio of two sums over the samples, both additive over batches;
+ * the paper names streaming as future work.  hcgrid_accumulate grids one batch
+ * (arguments as hcgrid_grid, DEVICE pointers, asynchronous on `stream`) and adds its
+ * un-normalised sums, weights and counts to accumulators owned by the context; the first call
+ * after hcgrid_set_target_* or after a resetting hcgrid_finalize starts from zero, and every
+ * batch of one accumulation must have the same nchan.  hcgrid_finalize writes
+ * datacube = sums / weightmap (NaN where the weight is 0), weightmap and, if not NULL, counts
+ * of everything accumulated so far; reset != 0 ends the accumulation.  Gridding batches one
+ * after the other equals gridding their union up to the order of the additions.
+ * hcgrid_set_target_* also ends a running accumulation. */
+int hcgrid_accumulate(hcgrid_ctx* ctx, int64_t n, const double* lon_deg, const double* lat_deg,
+                      const float* values, int32_t nchan, const float* weights, void* stream);
+int hcgrid_finalize(hcgrid_ctx* ctx, void* datacube, void* weightmap, int32_t* counts, int reset,
+                    void* stream);
+int64_t hcgrid_accumulated_batches(const hcgrid_ctx* ctx);   /* batches in the running accumulation */
+
 int64_t hcgrid_ncell(const hcgrid_ctx* ctx);      /* cells of the current target, 0 if none */
 int hcgrid_get_stats(const hcgrid_ctx* ctx, hcgrid_stats* out);
 const char* hcgrid_last_error(const hcgrid_ctx* ctx);  /* ctx may be NULL (create errors) */

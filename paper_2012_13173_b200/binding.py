@@ -26,7 +26,7 @@ EXPORTS = [
     "hcgrid_set_target_cells", "hcgrid_grid", "hcgrid_grid_host", "hcgrid_ncell",
     "hcgrid_get_stats", "hcgrid_last_error", "hcgrid_debug_preorder",
     "hcgrid_debug_ang2pix_ring", "hcgrid_host_ang2pix_ring", "hcgrid_host_ring_info",
-    "hcgrid_measure_peaks",
+    "hcgrid_measure_peaks", "hcgrid_accumulate", "hcgrid_finalize", "hcgrid_accumulated_batches",
 ]
 
 
@@ -70,6 +70,10 @@ def load_library():
     lib.hcgrid_set_target_cells.argtypes = [vp, i64, vp, vp, vp]
     lib.hcgrid_grid.argtypes = [vp, i64, vp, vp, vp, i32, vp, vp, vp, vp, vp]
     lib.hcgrid_grid_host.argtypes = [vp, i64, vp, vp, vp, i32, vp, vp, vp, vp]
+    lib.hcgrid_accumulate.argtypes = [vp, i64, vp, vp, vp, i32, vp, vp]
+    lib.hcgrid_finalize.argtypes = [vp, vp, vp, vp, ctypes.c_int, vp]
+    lib.hcgrid_accumulated_batches.argtypes = [vp]
+    lib.hcgrid_accumulated_batches.restype = i64
     lib.hcgrid_ncell.argtypes = [vp]
     lib.hcgrid_ncell.restype = i64
     lib.hcgrid_get_stats.argtypes = [vp, ctypes.POINTER(Stats)]
@@ -82,7 +86,7 @@ def load_library():
                                           ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
     lib.hcgrid_measure_peaks.argtypes = [ctypes.c_int, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
     for name in EXPORTS:
-        if name not in ("hcgrid_ncell", "hcgrid_last_error"):
+        if name not in ("hcgrid_ncell", "hcgrid_last_error", "hcgrid_accumulated_batches"):
             getattr(lib, name).restype = ctypes.c_int
     _lib = lib
     return lib
@@ -234,6 +238,52 @@ class HCGrid:
                 None if weights is None else weights.data_ptr(), cube.data_ptr(), wmap.data_ptr(),
                 None if cnt is None else cnt.data_ptr(), st))
         return cube, wmap, cnt
+
+    def accumulate(self, lon_deg, lat_deg, values, weights=None):
+        """hcgrid_accumulate: grid one batch (device tensors as in grid) and add its un-normalised
+        sums to the context's accumulators.  Asynchronous on torch's current stream."""
+        import torch
+        n = lon_deg.numel()
+        if values.dim() == 1:
+            values = values.view(n, 1)
+        nchan = values.shape[1]
+        for t, dt in ((lon_deg, torch.float64), (lat_deg, torch.float64), (values, torch.float32)):
+            if not (t.is_cuda and t.dtype == dt and t.is_contiguous()):
+                raise TypeError("accumulate wants contiguous CUDA tensors: lon/lat float64, values float32")
+        if lat_deg.numel() != n or values.shape[0] != n:
+            raise ValueError("lon, lat, values disagree on n")
+        if weights is not None and not (weights.is_cuda and weights.dtype == torch.float32
+                                        and weights.is_contiguous() and weights.numel() == n):
+            raise TypeError("weights must be a contiguous CUDA float32 tensor of n entries")
+        with torch.cuda.device(self.device):
+            st = torch.cuda.current_stream().cuda_stream
+            self._check(self._lib.hcgrid_accumulate(
+                self._ctx, n, lon_deg.data_ptr(), lat_deg.data_ptr(), values.data_ptr(), nchan,
+                None if weights is None else weights.data_ptr(), st))
+        self._acc_nchan = nchan
+
+    def finalize(self, want_counts: bool = True, reset: bool = True):
+        """hcgrid_finalize: (datacube, weightmap, counts or None) of everything accumulated."""
+        import torch
+        nchan = getattr(self, "_acc_nchan", 0)
+        if nchan == 0:
+            raise HCGridError(-2, "nothing accumulated")
+        odt = torch.float64 if self.precision == F64 else torch.float32
+        dev = torch.device("cuda", self.device)
+        cube = torch.empty((self.ncell, nchan), dtype=odt, device=dev)
+        wmap = torch.empty(self.ncell, dtype=odt, device=dev)
+        cnt = torch.empty(self.ncell, dtype=torch.int32, device=dev) if want_counts else None
+        with torch.cuda.device(self.device):
+            st = torch.cuda.current_stream().cuda_stream
+            self._check(self._lib.hcgrid_finalize(self._ctx, cube.data_ptr(), wmap.data_ptr(),
+                                                  None if cnt is None else cnt.data_ptr(), 1 if reset else 0, st))
+        if reset:
+            self._acc_nchan = 0
+        return cube, wmap, cnt
+
+    @property
+    def accumulated_batches(self) -> int:
+        return int(self._lib.hcgrid_accumulated_batches(self._ctx))
 
     def grid_host(self, lon_deg: np.ndarray, lat_deg: np.ndarray, values: np.ndarray,
                   weights: Optional[np.ndarray] = None, want_counts: bool = True, out=None):

@@ -85,7 +85,8 @@ int hcgrid_destroy(hcgrid_ctx* c) {
     DevBuf* bufs[] = {&c->d_strips, &c->d_wins, &c->d_winsf, &c->d_rowsf, &c->d_cell_lon, &c->d_cell_lat, &c->d_keys, &c->d_keys_out,
                       &c->d_idx, &c->d_idx_out, &c->d_sort_tmp, &c->d_bins, &c->d_rec, &c->d_misc,
                       &c->d_in_lon, &c->d_in_lat, &c->d_in_val, &c->d_in_wgt, &c->d_out_cube, &c->d_out_w,
-                      &c->d_out_cnt};
+                      &c->d_out_cnt, &c->d_acc_cube, &c->d_acc_w, &c->d_acc_cnt, &c->d_tmp_cube, &c->d_tmp_w,
+                      &c->d_tmp_cnt};
     for (DevBuf* b : bufs) b->release();
     for (auto& ev : c->ev) if (ev) cudaEventDestroy(ev);
     delete c;
@@ -138,6 +139,7 @@ int hcgrid_set_target_car(hcgrid_ctx* c, int32_t nx, int32_t ny, double lon0, do
         return fail(c, HCGRID_ERR_INVALID_ARG, "a target row must span less than 360 degrees");
     HCG_CUDA(c, cudaSetDevice(c->device));
     c->has_target = false;
+    c->acc_nchan = 0;
     return build_target_car(c, nx, ny, lon0, lat0, dlon, dlat);
 }
 
@@ -148,6 +150,7 @@ int hcgrid_set_target_cells(hcgrid_ctx* c, int64_t ncell, const double* lon, con
     if (!lon || !lat) return fail(c, HCGRID_ERR_INVALID_ARG, "lon_deg / lat_deg is NULL");
     HCG_CUDA(c, cudaSetDevice(c->device));
     c->has_target = false;
+    c->acc_nchan = 0;
     return build_target_cells(c, ncell, lon, lat, (cudaStream_t)stream);
 }
 

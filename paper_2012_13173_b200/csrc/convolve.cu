@@ -294,6 +294,7 @@ int run_convolve(hcgrid_ctx* c, int64_t n, const float* values, int nchan, bool 
     a.rg = rg; a.kp = c->kp;
     a.kmax = c->kmax; a.strip_cells = c->strip_cells;
     a.nchan = nchan;
+    a.raw = c->raw_sums ? 1 : 0;
     a.qx = (float)(1.0 / rg.sx32);
     a.qy = (float)(1.0 / rg.sy32);
     a.sx = rg.sx32;
@@ -314,7 +315,7 @@ int run_convolve(hcgrid_ctx* c, int64_t n, const float* values, int nchan, bool 
     } else if (f32 && nchan == 1 && c->tile_ok && (c->opt_kernel == 0 || c->opt_kernel == 5)) {
         rc = launch_conv_tile(c, n, (float*)cube, (float*)wmap, counts, st);
         c->stats.kernel = 6;
-    } else if (f32 && nchan == 1 && c->opt_kernel != 3) {
+    } else if (f32 && nchan == 1 && c->opt_kernel != 3 && !c->raw_sums) {
         const bool staged = c->opt_kernel != 1 && c->kmax <= 32;
         int G = c->opt_coarsen;
         if (G == 0) G = c->strip_cells >= 4 ? 2 : 1;

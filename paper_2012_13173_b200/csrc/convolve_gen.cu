@@ -135,7 +135,7 @@ conv_general(const ConvArgs a) {
         const AccT nan = NanOf<AccT>::v();
         if (nchan == 1) {
             const AccT S = warp_sum(acc[0]);
-            if (lane == 0) cube[task] = W > (AccT)0 ? S / W : nan;
+            if (lane == 0) cube[task] = a.raw ? S : (W > (AccT)0 ? S / W : nan);
         } else if (VEC4) {
 #pragma unroll
             for (int j = 0; j < 2; ++j) {
@@ -143,14 +143,14 @@ conv_general(const ConvArgs a) {
                 if (c < nchan) {
                     AccT* o = cube + (size_t)task * nchan + c;
 #pragma unroll
-                    for (int t = 0; t < 4; ++t) o[t] = W > (AccT)0 ? acc[4 * j + t] / W : nan;
+                    for (int t = 0; t < 4; ++t) o[t] = a.raw ? acc[4 * j + t] : (W > (AccT)0 ? acc[4 * j + t] / W : nan);
                 }
             }
         } else {
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
                 const int c = ch0 + lane + 32 * j;
-                if (c < nchan) cube[(size_t)task * nchan + c] = W > (AccT)0 ? acc[j] / W : nan;
+                if (c < nchan) cube[(size_t)task * nchan + c] = a.raw ? acc[j] : (W > (AccT)0 ? acc[j] / W : nan);
             }
         }
         if (ch0 == 0 && lane == 0) {

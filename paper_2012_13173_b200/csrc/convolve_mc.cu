@@ -329,7 +329,7 @@ conv_mc_f32(const McArgs m) {
                 for (int k = 0; k < 4; ++k) unpack2(acc[c][k], f[2 * k], f[2 * k + 1]);
                 const float nan = __int_as_float(0x7fc00000);
 #pragma unroll
-                for (int k = 0; k < 8; ++k) f[k] = wc > 0.0f ? f[k] / wc : nan;
+                for (int k = 0; k < 8; ++k) f[k] = a.raw ? f[k] : (wc > 0.0f ? f[k] / wc : nan);
                 if (ok0) *(float4*)o = make_float4(f[0], f[1], f[2], f[3]);
                 if (ok1) *(float4*)(o + 4) = make_float4(f[4], f[5], f[6], f[7]);
             }

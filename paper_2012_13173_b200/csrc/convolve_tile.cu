@@ -179,7 +179,7 @@ conv1_tile_f32(const TileArgs a) {
         const int gx = c % GX, gy = c / GX;
         if (gx < ncols && gy < nrows) {
             const int64_t cell = (int64_t)(row0 + gy) * a.nx + ix0 + gx;
-            a.cube[cell] = wsum > 0.0f ? ssum / wsum : __int_as_float(0x7fc00000);
+            a.cube[cell] = a.raw ? ssum : (wsum > 0.0f ? ssum / wsum : __int_as_float(0x7fc00000));
             a.wmap[cell] = wsum;
             if (COUNTS) a.counts[cell] = csum;
         }
@@ -251,6 +251,7 @@ void fill_tile_args(const hcgrid_ctx* c, int mode, TileArgs& a) {
     a.a12 = (float)(1.0 / (12.0 * kappa));
     a.hmax = (float)(mode == 0 ? kappa * kp.radius * kp.radius : kappa * 4.0 * kp.hav_max);
     a.split = 1;
+    a.raw = c->raw_sums ? 1 : 0;
 }
 
 int launch_conv_tile(hcgrid_ctx* c, int64_t n, float* cube, float* wmap, int32_t* counts, cudaStream_t st) {

@@ -146,6 +146,11 @@ struct hcgrid_ctx {
     // per-call scratch
     hcg::DevBuf d_keys, d_keys_out, d_idx, d_idx_out, d_sort_tmp, d_bins, d_rec, d_misc;
     hcg::DevBuf d_in_lon, d_in_lat, d_in_val, d_in_wgt, d_out_cube, d_out_w, d_out_cnt;  // *_host path
+    // incremental gridding (hcgrid_accumulate / hcgrid_finalize): un-normalised sums over the batches so far
+    hcg::DevBuf d_acc_cube, d_acc_w, d_acc_cnt, d_tmp_cube, d_tmp_w, d_tmp_cnt;
+    bool raw_sums = false;          // the convolution kernels write sums instead of sums / W
+    int acc_nchan = 0;              // channels of the running accumulation (0: none yet)
+    int64_t acc_batches = 0;
     // last call (debug introspection)
     const double* last_lon = nullptr;
     const double* last_lat = nullptr;

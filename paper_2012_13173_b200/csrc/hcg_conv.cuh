@@ -21,6 +21,7 @@ struct ConvArgs {
     int64_t ntasks;
     int32_t nchan;
     int32_t chunk;              // records per staging buffer (staged kernel)
+    int32_t raw;                // 1: write the un-normalised sums (incremental gridding)
     float qx, qy;               // radians per fixed-point unit
     double sx;                  // fixed-point units per radian (lon)
 };

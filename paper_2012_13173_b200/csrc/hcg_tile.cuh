@@ -17,6 +17,7 @@ struct TileArgs {
     double u0, du, sx;          // lon offset of column 0 (rad), column step (rad), fixed-point units per rad
     int32_t nx, ny, kmax, m;    // target shape, window-table row length, lookup bins per ring
     int32_t tiles_x;
+    int32_t raw;                // 1: write the un-normalised sums (incremental gridding), 0: sums / W
     int32_t split;              // warps per tile (1, 2, 4 or 8): long candidate streams of few tiles are split
     int64_t ntiles;
     float sxk, syk;             // sqrt(kappa) * radians per fixed-point unit (lon, lat)

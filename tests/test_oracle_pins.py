@@ -227,3 +227,30 @@ def test_duplicates_all_count(oracle):
     assert r.counts[0] == 4
     assert r.datacube[0, 0] == pytest.approx(3.0, rel=1e-15)
     assert r.weightmap[0] == pytest.approx(4 * math.exp(-0.5 * 0.25), rel=1e-14)
+
+
+def test_batches_are_additive_in_the_unnormalised_sums(oracle):
+    """Eq. 1 is a ratio of two sums over the samples, so gridding two batches and
+    combining  V = (V_a W_a + V_b W_b) / (W_a + W_b),  W = W_a + W_b,  counts added,  must equal
+    gridding their union (the semantics of incremental gridding, hcgrid_accumulate)."""
+    rng = np.random.default_rng(31)
+    n = 900
+    lon = 10.0 + rng.uniform(-0.2, 0.2, n)
+    lat = -30.0 + rng.uniform(-0.2, 0.2, n)
+    val = rng.normal(size=(n, 3)).astype(np.float32)
+    wts = rng.uniform(0.5, 1.5, n).astype(np.float32)
+    gx, gy = np.meshgrid(10.0 + np.linspace(-0.45, 0.45, 9), -30.0 + np.linspace(-0.45, 0.45, 8))
+    cl, cb = gx.ravel(), gy.ravel()
+    sigma, radius = 2.0 / 60.0, 6.0 / 60.0
+    cut = 350
+    full = oracle.grid(sigma, radius, cl, cb, lon, lat, val, wts)
+    a = oracle.grid(sigma, radius, cl, cb, lon[:cut], lat[:cut], val[:cut], wts[:cut])
+    b = oracle.grid(sigma, radius, cl, cb, lon[cut:], lat[cut:], val[cut:], wts[cut:])
+    w = a.weightmap + b.weightmap
+    s = np.nan_to_num(a.datacube) * a.weightmap[:, None] + np.nan_to_num(b.datacube) * b.weightmap[:, None]
+    with np.errstate(invalid="ignore", divide="ignore"):
+        v = np.where(w[:, None] > 0, s / w[:, None], np.nan)
+    assert np.array_equal(a.counts + b.counts, full.counts)
+    np.testing.assert_allclose(w, full.weightmap, rtol=1e-13)
+    np.testing.assert_allclose(v, full.datacube, rtol=1e-11, atol=1e-13, equal_nan=True)
+    assert (full.weightmap == 0).any() and (full.weightmap > 0).any()      # the case has empty cells too

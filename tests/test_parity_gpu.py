@@ -568,3 +568,31 @@ def wl_like(tgt, lon, lat, val, wts, sigma, radius, nside=2048):
     w.lon, w.lat, w.values, w.weights, w.target = lon, lat, val, wts, tgt
     w.sigma_deg, w.radius_deg, w.nside = sigma, radius, nside
     return w
+
+
+# ------------------------------------------------------------ incremental gridding
+@pytest.mark.parametrize("cfg,precision", [(1, "f32"), (3, "f32"), (5, "f32"), (4, "f32"), (2, "f64")])
+def test_accumulate_batches_equal_the_union(oracle, cfg, precision):
+    """hcgrid_accumulate over uneven batches (one of them empty) + hcgrid_finalize against the
+    oracle on ALL samples; a second accumulation on the same context starts from zero."""
+    from paper_2012_13173_b200 import binding
+    w, ref = mini(oracle, cfg)
+    t = w.target
+    tol = TOL_F32 if precision == "f32" else TOL_F64
+    g = binding.HCGrid(w.sigma_deg, w.radius_deg, w.nside, precision=precision)
+    g.set_target_car(t.nx, t.ny, t.lon0, t.lat0, t.dlon, t.dlat)
+    lon, lat, val = _dev(w.lon), _dev(w.lat), _dev(w.values)
+    wts = None if w.weights is None else _dev(w.weights)
+    cuts = [0, w.n // 5, w.n // 5, w.n // 2 + 7, w.n]
+    for rep in range(2):
+        for a, b in zip(cuts[:-1], cuts[1:]):
+            g.accumulate(lon[a:b].contiguous(), lat[a:b].contiguous(), val[a:b].contiguous(),
+                         None if wts is None else wts[a:b].contiguous())
+        assert g.accumulated_batches == 4
+        cube, wmap, cnt = g.finalize(reset=True)
+        torch.cuda.synchronize()
+        assert g.accumulated_batches == 0
+        compare(cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy(), ref, w.sigma_deg, w.radius_deg, tol, qmax(w))
+    with pytest.raises(binding.HCGridError):
+        g.finalize()
+    g.close()
