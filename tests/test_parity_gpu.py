@@ -596,3 +596,41 @@ def test_accumulate_batches_equal_the_union(oracle, cfg, precision):
     with pytest.raises(binding.HCGridError):
         g.finalize()
     g.close()
+
+
+def test_context_reuse_streams_and_retargeting(oracle):
+    """One context through: a call on a non-default stream, a larger call (scratch grows), a new
+    target, and a smaller call again -- each checked against the oracle."""
+    from paper_2012_13173_b200 import binding
+    w1, ref1 = mini(oracle, 1)
+    w3, ref3 = mini(oracle, 3)
+    g = binding.HCGrid(w1.sigma_deg, w1.radius_deg, w1.nside)
+    t = w1.target
+    g.set_target_car(t.nx, t.ny, t.lon0, t.lat0, t.dlon, t.dlat)
+    side = torch.cuda.Stream()
+    half = w1.n // 2
+    lon, lat, val = _dev(w1.lon), _dev(w1.lat), _dev(w1.values)
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        cube_h, wmap_h, cnt_h = g.grid(lon[:half].contiguous(), lat[:half].contiguous(), val[:half].contiguous())
+    side.synchronize()
+    ref_h = oracle.grid(w1.sigma_deg, w1.radius_deg, *t.cell_centers(), w1.lon[:half], w1.lat[:half], w1.values[:half])
+    compare(cube_h.cpu().numpy(), wmap_h.cpu().numpy(), cnt_h.cpu().numpy(), ref_h, w1.sigma_deg, w1.radius_deg, TOL_F32)
+    cube, wmap, cnt = g.grid(lon, lat, val)                  # larger n: scratch grows
+    torch.cuda.synchronize()
+    compare(cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy(), ref1, w1.sigma_deg, w1.radius_deg, TOL_F32)
+    g.close()
+    # same kernel parameters as config 3, two targets in turn on one context
+    g = binding.HCGrid(w3.sigma_deg, w3.radius_deg, w3.nside)
+    t3 = w3.target
+    g.set_target_car(5, 4, t3.lon0, t3.lat0, t3.dlon, t3.dlat)
+    small = g.grid(_dev(w3.lon), _dev(w3.lat), _dev(w3.values))
+    g.set_target_car(t3.nx, t3.ny, t3.lon0, t3.lat0, t3.dlon, t3.dlat)
+    cube, wmap, cnt = g.grid(_dev(w3.lon), _dev(w3.lat), _dev(w3.values))
+    torch.cuda.synchronize()
+    compare(cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy(), ref3, w3.sigma_deg, w3.radius_deg, TOL_F32)
+    # the 5 x 4 corner of the big target must agree with the small target's result bit for bit or to tolerance
+    idx = (np.arange(4)[:, None] * t3.nx + np.arange(5)[None, :]).ravel()
+    np.testing.assert_allclose(small[1].cpu().numpy(), wmap.cpu().numpy()[idx], rtol=2e-6)
+    assert np.array_equal(small[2].cpu().numpy(), cnt.cpu().numpy()[idx])
+    g.close()
