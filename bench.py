@@ -178,6 +178,17 @@ def run_product(args):
     # every rank grids one independent, identically shaped problem (weak scaling; the path has no
     # data-path collective: DESIGN.md "Multi-GPU")
     w = workloads.make(args.config, args.scale)
+    units_total = None
+    if args.shard == "rows" and world > 1:
+        # strong scaling: ONE problem, every rank owns a band of target rows and the samples within the
+        # support radius of it (paper_2012_13173_b200/dist.py); outputs are disjoint, no collective
+        full = w.target
+        units_total = full.ncell * w.nchan
+        iy0, iy1 = hdist.row_band(full.ny, world, rank, align=4)
+        m = hdist.band_sample_mask(w.lat, full, iy0, iy1, w.radius_deg)
+        w.target = hdist.band_target(full, iy0, iy1)
+        w.lon, w.lat, w.values = w.lon[m], w.lat[m], np.ascontiguousarray(w.values[m])
+        w.weights = None if w.weights is None else w.weights[m]
     t = w.target
     g = binding.HCGrid(w.sigma_deg, w.radius_deg, w.nside, precision="f32", device=local)
     g.set_target_car(t.nx, t.ny, t.lon0, t.lat0, t.dlon, t.dlat)
@@ -266,8 +277,12 @@ def run_product(args):
             dist.destroy_process_group()
         return 0
 
-    units = ncell * nchan * world
-    value = hdist.whole_job_rate(ncell * nchan, world, args.steps, ms_total)
+    if units_total is None:
+        units = ncell * nchan * world
+        value = hdist.whole_job_rate(ncell * nchan, world, args.steps, ms_total)
+    else:
+        units = units_total
+        value = units_total * args.steps / (ms_total * 1e-3)
     hbm_gbs, hbm_src = load_peaks()
     t_conv = float(np.mean(stage["us_convolve"])) * 1e-6
     cand = roofline.count_candidates(w, max_rows=args.cand_rows)
@@ -319,12 +334,12 @@ def run_product(args):
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "scaling": "weak" if units_total is None else "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": WORKLOAD_NAMES[args.config], "scale": args.scale, "n_samples": w.n, "ncell": ncell,
                    "nchan": nchan, "nside": w.nside, "sigma_arcmin": w.sigma_deg * 60, "radius_arcmin": w.radius_deg * 60,
                    "l2": "inputs larger than L2 (no flush): lon/lat/values %.0f MB + packed records %.0f MB per step"
                          % (h2d / 1e6, st["n_kept"] * 16 / 1e6),
-                   "coarsen": st["coarsen"], "coarsen_y": st["coarsen_y"], "subpix_bits": st["subpix_bits"], "per_rank": "one independent problem",
+                   "coarsen": st["coarsen"], "coarsen_y": st["coarsen_y"], "subpix_bits": st["subpix_bits"], "per_rank": "one independent problem" if units_total is None else "a band of target rows + its samples (rank 0's figures in roofline / stages)",
                    "outputs": "datacube + weight map (count output off in the timed calls)"},
         "kernel_evals_per_s": n_hit * world * args.steps / (ms_total * 1e-3),
         "conv_kernel": {"us": t_conv * 1e6, "cell_channels_per_s": ncell * nchan / t_conv,
@@ -356,6 +371,8 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cand-rows", type=int, default=None, help="count N_cand on this many rows and scale")
+    ap.add_argument("--shard", default="replicas", choices=["replicas", "rows"],
+                    help="N > 1: independent replicas (weak scaling, default) or one problem cut into row bands (strong)")
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per launch of the convolution kernel from the committed ncu capture")
     args = ap.parse_args()

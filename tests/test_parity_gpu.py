@@ -634,3 +634,24 @@ def test_context_reuse_streams_and_retargeting(oracle):
     np.testing.assert_allclose(small[1].cpu().numpy(), wmap.cpu().numpy()[idx], rtol=2e-6)
     assert np.array_equal(small[2].cpu().numpy(), cnt.cpu().numpy()[idx])
     g.close()
+
+
+def test_row_band_sharding_on_one_gpu(oracle):
+    """The multi-GPU row-band sharding (dist.py), its ranks run one after the other on this GPU:
+    the concatenated bands match the oracle on the whole target."""
+    from paper_2012_13173_b200 import binding, dist as hdist
+    w, ref = mini(oracle, 3)
+    t = w.target
+    world = 3
+    cubes, wmaps, cnts = [], [], []
+    for r in range(world):
+        a, b = hdist.row_band(t.ny, world, r, align=4)
+        bt = hdist.band_target(t, a, b)
+        m = hdist.band_sample_mask(w.lat, t, a, b, w.radius_deg)
+        g = binding.HCGrid(w.sigma_deg, w.radius_deg, w.nside)
+        g.set_target_car(bt.nx, bt.ny, bt.lon0, bt.lat0, bt.dlon, bt.dlat)
+        cube, wmap, cnt = g.grid(_dev(w.lon[m]), _dev(w.lat[m]), _dev(np.ascontiguousarray(w.values[m])))
+        torch.cuda.synchronize()
+        cubes.append(cube.cpu().numpy()); wmaps.append(wmap.cpu().numpy()); cnts.append(cnt.cpu().numpy())
+        g.close()
+    compare(np.concatenate(cubes), np.concatenate(wmaps), np.concatenate(cnts), ref, w.sigma_deg, w.radius_deg, TOL_F32)
