@@ -22,6 +22,7 @@ struct ConvArgs {
     int32_t nchan;
     int32_t chunk;              // records per staging buffer (staged kernel)
     int32_t raw;                // 1: write the un-normalised sums (incremental gridding)
+    int32_t small64;            // 1: fp64 pairs by the small-angle series (pair64_small), 0: full functions
     float qx, qy;               // radians per fixed-point unit
     double sx;                  // fixed-point units per radian (lon)
 };
