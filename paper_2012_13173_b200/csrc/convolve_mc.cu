@@ -274,15 +274,16 @@ conv_mc_f32(const McArgs m) {
                             issue(ent_s + (kRowDepth - 1) * (kHitStride * 4),
                                   vring + (uint32_t)((e + kRowDepth - 1) & (kRowDepth - 1)) * 1024u);
                         cp_async_commit();
+                        // the 8 weights by two broadcast loads, issued before the wait for the row so that
+                        // their latency hides behind it; each weight is paired with itself in registers
+                        // (duplicated pairs in shared memory cost twice the load/store-pipe cycles)
+                        const float4 wlo = lds128(ent_s), whi = lds128(ent_s + 16);
                         cp_async_wait<kRowDepth - 1>();     // row e has landed (each lane reads its own bytes)
                         const uint32_t src = vring + (uint32_t)(e & (kRowDepth - 1)) * 1024u;
                         // lanes past nchan read stale shared memory: their sums are never stored
                         const float4 va = lds128(src), vb = lds128(src + 16);
                         const unsigned long long v01 = pack2(va.x, va.y), v23 = pack2(va.z, va.w);
                         const unsigned long long v45 = pack2(vb.x, vb.y), v67 = pack2(vb.z, vb.w);
-                        // the 8 weights by two broadcast loads; each is paired with itself in registers
-                        // (duplicated pairs in shared memory cost twice the load/store-pipe cycles)
-                        const float4 wlo = lds128(ent_s), whi = lds128(ent_s + 16);
                         const float wv[8] = {wlo.x, wlo.y, wlo.z, wlo.w, whi.x, whi.y, whi.z, whi.w};
 #pragma unroll
                         for (int c = 0; c < 8; ++c) {
