@@ -68,7 +68,9 @@ enum {
                                     6 = force the cube kernel (nchan > 1; error if not applicable) */
     HCGRID_OPT_WARPS_PER_SM = 5, /* resident convolution warps per SM (staged kernel); 0 = auto */
     HCGRID_OPT_COARSEN_Y = 6,    /* target rows per warp task (tile kernel); 0 = auto */
-    HCGRID_OPT_SPLIT = 7         /* warps sharing one tile's candidate stream (tile kernel): 1, 2, 4; 0 = auto */
+    HCGRID_OPT_SPLIT = 7,        /* warps sharing one tile's candidate stream (tile kernel): 1, 2, 4; 0 = auto */
+    HCGRID_OPT_PREORDER = 8      /* how S' is ordered: 1 = radix sort of (key, n); 2 = counting sort into the
+                                    bin table (same S', bit for bit); 0 = auto (counting unless n >> bins) */
 };
 
 typedef struct {
@@ -83,7 +85,7 @@ typedef struct {
     int32_t coarsen_y;        /* target rows per warp task used (tile kernel; else 1)         */
     float us_pixelise, us_sort, us_tables, us_pack, us_convolve, us_total; /* PROFILE only   */
     int32_t split;            /* warps per tile used (tile kernel; else 1)                    */
-    int32_t reserved;
+    int32_t preorder;         /* pre-ordering used: 1 radix sort, 2 counting sort             */
 } hcgrid_stats;
 
 /* Create a context.  sigma_deg = kernel standard deviation, support_radius_deg =

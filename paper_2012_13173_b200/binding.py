@@ -18,7 +18,8 @@ _LIB_PATH = os.path.join(_HERE, "libhcgrid.so")
 _lib = None
 
 F32, F64 = 0, 1
-OPT_PROFILE, OPT_SUBPIX_BITS, OPT_COARSEN, OPT_KERNEL, OPT_WARPS_PER_SM, OPT_COARSEN_Y, OPT_SPLIT = 1, 2, 3, 4, 5, 6, 7
+OPT_PROFILE, OPT_SUBPIX_BITS, OPT_COARSEN, OPT_KERNEL, OPT_WARPS_PER_SM, OPT_COARSEN_Y, OPT_SPLIT, OPT_PREORDER = 1, 2, 3, 4, 5, 6, 7, 8
+PREORDER_AUTO, PREORDER_RADIX, PREORDER_COUNTING = 0, 1, 2
 KERNEL_AUTO, KERNEL_SIMPLE, KERNEL_F64PAIR, KERNEL_GENERAL, KERNEL_STAGED, KERNEL_TILE, KERNEL_CUBE = 0, 1, 2, 3, 4, 5, 6
 
 EXPORTS = [
@@ -42,7 +43,7 @@ class Stats(ctypes.Structure):
                 ("kernel", ctypes.c_int32), ("gpu_launches", ctypes.c_int32), ("coarsen_y", ctypes.c_int32),
                 ("us_pixelise", ctypes.c_float), ("us_sort", ctypes.c_float), ("us_tables", ctypes.c_float),
                 ("us_pack", ctypes.c_float), ("us_convolve", ctypes.c_float), ("us_total", ctypes.c_float),
-                ("split", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+                ("split", ctypes.c_int32), ("preorder", ctypes.c_int32)]
 
     def asdict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

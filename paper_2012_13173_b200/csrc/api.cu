@@ -122,6 +122,10 @@ int hcgrid_set_option(hcgrid_ctx* c, int option, int64_t value) {
                 return fail(c, HCGRID_ERR_INVALID_ARG, "split must be 0 (auto), 1, 2 or 4");
             c->opt_split = (int)value;
             break;
+        case HCGRID_OPT_PREORDER:
+            if (value < 0 || value > 2) return fail(c, HCGRID_ERR_INVALID_ARG, "preorder must be 0 (auto), 1 or 2");
+            c->opt_preorder = (int)value;
+            break;
         default: return fail(c, HCGRID_ERR_INVALID_ARG, "unknown option %d", option);
     }
     return HCGRID_OK;

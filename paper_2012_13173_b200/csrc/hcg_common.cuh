@@ -129,7 +129,7 @@ struct hcgrid_ctx {
     int num_sms = 148;
     hcg::KernelParams kp{};
     // options
-    int opt_profile = 0, opt_subpix = -1000, opt_coarsen = 0, opt_coarsen_y = 0, opt_kernel = 0, opt_warps = 0, opt_split = 0;
+    int opt_profile = 0, opt_subpix = -1000, opt_coarsen = 0, opt_coarsen_y = 0, opt_kernel = 0, opt_warps = 0, opt_split = 0, opt_preorder = 0;
     // target
     bool has_target = false;
     bool is_car = false;

@@ -16,17 +16,20 @@
 //                 fixed-point records (fp32 mode) or degree records (fp64 mode).  In fp32
 //                 mode a4 and a5 are one kernel: one pass over the sorted pairs.
 #include <cub/device/device_radix_sort.cuh>
+#include <cub/device/device_scan.cuh>
 
 #include "hcg_common.cuh"
 
 namespace hcg {
 
-template <bool kF32>
+// kCount: the counting pre-order (below) -- idx[i] receives the sample's arrival rank within
+// its bin (global atomic on the bin's counter) instead of i.
+template <bool kF32, bool kCount>
 __global__ void __launch_bounds__(256)
 pixelise_kernel(const double* __restrict__ lon_deg, const double* __restrict__ lat_deg,
                 const float* __restrict__ values, const float* __restrict__ weights,
                 int nchan, int64_t n, Region rg, uint32_t* __restrict__ keys,
-                uint32_t* __restrict__ idx, Rec32* __restrict__ rec) {
+                uint32_t* __restrict__ idx, Rec32* __restrict__ rec, int32_t* __restrict__ bin_count) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const double lo_d = lon_deg[i], la_d = lat_deg[i];
@@ -61,7 +64,8 @@ pixelise_kernel(const double* __restrict__ lon_deg, const double* __restrict__ l
         }
     }
     keys[i] = key;
-    idx[i] = (uint32_t)i;
+    if (kCount) idx[i] = key != (uint32_t)rg.nbins ? (uint32_t)atomicAdd(bin_count + key, 1) : 0u;
+    else idx[i] = (uint32_t)i;
     if (kF32) {
         if (nchan == 1) r.v = values[i];
         if (weights) r.q = weights[i];
@@ -108,13 +112,109 @@ tables_pack_kernel(const uint32_t* __restrict__ skeys, const uint32_t* __restric
     }
 }
 
+// ---- counting pre-order: a3..a5 without the multi-pass radix sort -------------------
+// The keys are bin numbers of a table that is built anyway, so the sort of PAPER.md:120 is a
+// counting sort: pixelise_kernel<.., true> counts every bin and keeps each sample's arrival
+// rank, an exclusive scan of the counts IS bin_start (a4), scatter_index_kernel puts sample i
+// at bin_start[key] + rank, and bin_order_kernel puts every bin's indices in ascending order
+// -- arrival order is whatever the atomics made it; ascending index is what the stable sort
+// gives, so S' is identical to the radix path's, bit for bit.  pack32_kernel gathers (a5).
+
 __global__ void __launch_bounds__(256)
-pack64_kernel(const uint32_t* __restrict__ skeys, const uint32_t* __restrict__ sidx, int64_t n,
-              uint32_t sentinel, const double* __restrict__ lon_deg, const double* __restrict__ lat_deg,
-              const float* __restrict__ weights, Rec64* __restrict__ rec_out) {
+scatter_index_kernel(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ rank, int64_t n,
+                     int32_t nbins, const int32_t* __restrict__ bin_start, uint32_t* __restrict__ sidx) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    if (skeys[i] == sentinel) return;
+    const uint32_t key = keys[i];
+    if (key >= (uint32_t)nbins) return;
+    sidx[(int64_t)__ldg(bin_start + key) + rank[i]] = (uint32_t)i;
+}
+
+// Ascending sort of a[0, L) by the whole block, in place in global memory: the bitonic
+// network in its all-ascending form (first sub-stage of every stage mirrors, the others
+// shift), so the virtual padding to a power of two sits at the top and is never touched.
+__device__ __forceinline__ void cmp_swap(uint32_t* a, int i, int j, int L) {
+    if (j < L) {
+        const uint32_t x = a[i], y = a[j];
+        if (x > y) { a[i] = y; a[j] = x; }
+    }
+}
+
+__device__ void block_sort_u32(uint32_t* a, int L, int tid, int nthr) {
+    int P = 1;
+    while (P < L) P <<= 1;
+    for (int k = 2; k <= P; k <<= 1) {
+        for (int t = tid; t < P / 2; t += nthr) {
+            const int l = t & (k / 2 - 1), base = (t - l) * 2;
+            cmp_swap(a, base + l, base + k - 1 - l, L);
+        }
+        __syncthreads();
+        for (int j = k >> 2; j >= 1; j >>= 1) {
+            for (int t = tid; t < P / 2; t += nthr) {
+                const int l = t & (j - 1), i = (t - l) * 2 + l;
+                cmp_swap(a, i, i + j, L);
+            }
+            __syncthreads();
+        }
+    }
+}
+
+constexpr int kThreadSortMax = 12;   // longer bins are sorted by the whole block
+
+// Thread b owns bin b: orders sidx[bin_start[b], bin_start[b+1]) ascending.  Bins longer than
+// kThreadSortMax are queued in shared memory and sorted by the whole block (rare unless
+// samples pile up in one place).
+__global__ void __launch_bounds__(256)
+bin_order_kernel(int32_t nbins, const int32_t* __restrict__ bin_start, uint32_t* sidx) {
+    __shared__ int s_cnt;
+    __shared__ int s_lo[256], s_len[256];
+    const int tid = threadIdx.x;
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + tid;
+    if (tid == 0) s_cnt = 0;
+    __syncthreads();
+    if (b < nbins) {
+        const int s = bin_start[b], e = bin_start[b + 1];
+        const int cnt = e - s;
+        if (cnt > kThreadSortMax) {
+            const int slot = atomicAdd(&s_cnt, 1);
+            s_lo[slot] = s; s_len[slot] = cnt;
+        } else if (cnt == 2) {
+            const uint32_t x = sidx[s], y = sidx[s + 1];
+            if (x > y) { sidx[s] = y; sidx[s + 1] = x; }
+        } else if (cnt > 2) {
+            for (int a = s + 1; a < e; ++a) {               // insertion sort, in place
+                const uint32_t v = sidx[a];
+                int p = a;
+                while (p > s) {
+                    const uint32_t u = sidx[p - 1];
+                    if (u <= v) break;
+                    sidx[p] = u;
+                    --p;
+                }
+                sidx[p] = v;
+            }
+        }
+    }
+    __syncthreads();
+    const int nq = s_cnt;
+    for (int g = 0; g < nq; ++g) block_sort_u32(sidx + s_lo[g], s_len[g], tid, 256);
+}
+
+// a5 after the counting sort: rec_out[p] = rec_in[sidx[p]] for p < nkept = bin_start[nbins].
+__global__ void __launch_bounds__(256)
+pack32_kernel(const uint32_t* __restrict__ sidx, int64_t n, const int32_t* __restrict__ nkept,
+              const Rec32* __restrict__ rec_in, Rec32* __restrict__ rec_out) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n || i >= (int64_t)nkept[0]) return;
+    *(uint4*)(rec_out + i) = __ldg((const uint4*)(rec_in + sidx[i]));
+}
+
+__global__ void __launch_bounds__(256)
+pack64_kernel(const uint32_t* __restrict__ sidx, int64_t n, const int32_t* __restrict__ nkept,
+              const double* __restrict__ lon_deg, const double* __restrict__ lat_deg,
+              const float* __restrict__ weights, Rec64* __restrict__ rec_out) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n || i >= (int64_t)nkept[0]) return;          // nkept = bin_start[nbins]
     const uint32_t s = sidx[i];
     Rec64 r;
     r.lon_deg = lon_deg[s];
@@ -129,9 +229,11 @@ int run_preorder(hcgrid_ctx* c, int64_t n, const double* lon, const double* lat,
                  int nchan, const float* weights, cudaStream_t st) {
     const Region& rg = c->region;
     const bool f32 = c->precision == HCGRID_F32 && c->f32_series_ok && c->opt_kernel != 2;
+    // counting pre-order unless the samples pile up (long bins, contended counters) or the
+    // option says otherwise; the result is the same S' either way
+    const bool counting = n > 0 && (c->opt_preorder == 2 || (c->opt_preorder == 0 && n <= 4 * (int64_t)rg.nbins && (int64_t)rg.nbins <= 16 * n));
     const size_t nn = (size_t)(n > 0 ? n : 1);
     HCG_CUDA(c, c->d_keys.ensure(nn * 4));
-    HCG_CUDA(c, c->d_keys_out.ensure(nn * 4));
     HCG_CUDA(c, c->d_idx.ensure(nn * 4));
     HCG_CUDA(c, c->d_idx_out.ensure(nn * 4));
     HCG_CUDA(c, c->d_bins.ensure(((size_t)rg.nbins + 2) * 4));
@@ -140,49 +242,86 @@ int run_preorder(hcgrid_ctx* c, int64_t n, const double* lon, const double* lat,
     int end_bit = 1;
     while (end_bit < 32 && ((uint64_t)1 << end_bit) <= (uint64_t)rg.nbins) ++end_bit;
     size_t tmp_bytes = 0;
-    HCG_CUDA(c, cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, c->d_keys.as<uint32_t>(),
-                                                c->d_keys_out.as<uint32_t>(), c->d_idx.as<uint32_t>(),
-                                                c->d_idx_out.as<uint32_t>(), (int64_t)nn, 0, end_bit, st));
+    if (counting) {
+        HCG_CUDA(c, cub::DeviceScan::ExclusiveSum(nullptr, tmp_bytes, c->d_bins.as<int32_t>(), c->d_bins.as<int32_t>(),
+                                                  (int64_t)rg.nbins + 1, st));
+    } else {
+        HCG_CUDA(c, c->d_keys_out.ensure(nn * 4));
+        HCG_CUDA(c, cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, c->d_keys.as<uint32_t>(),
+                                                    c->d_keys_out.as<uint32_t>(), c->d_idx.as<uint32_t>(),
+                                                    c->d_idx_out.as<uint32_t>(), (int64_t)nn, 0, end_bit, st));
+    }
     HCG_CUDA(c, c->d_sort_tmp.ensure(tmp_bytes + 16));
 
     const int threads = 256;
     const unsigned nb = (unsigned)((nn + threads - 1) / threads);
     int launches = 0;
+    c->stats.preorder = counting ? 2 : 1;
     if (c->opt_profile) cudaEventRecord(c->ev[0], st);
-    if (n > 0) {
+    if (counting) {
+        int32_t* bins = c->d_bins.as<int32_t>();
+        uint32_t* keys = c->d_keys.as<uint32_t>();
+        uint32_t* rank = c->d_idx.as<uint32_t>();
+        uint32_t* sidx = c->d_idx_out.as<uint32_t>();
+        HCG_CUDA(c, cudaMemsetAsync(bins, 0, ((size_t)rg.nbins + 1) * 4, st));
         if (f32)
-            pixelise_kernel<true><<<nb, threads, 0, st>>>(lon, lat, values, weights, nchan, n, rg,
-                                                          c->d_keys.as<uint32_t>(), c->d_idx.as<uint32_t>(),
-                                                          c->d_misc.as<Rec32>());
+            pixelise_kernel<true, true><<<nb, threads, 0, st>>>(lon, lat, values, weights, nchan, n, rg, keys, rank,
+                                                                c->d_misc.as<Rec32>(), bins);
         else
-            pixelise_kernel<false><<<nb, threads, 0, st>>>(lon, lat, values, weights, nchan, n, rg,
-                                                           c->d_keys.as<uint32_t>(), c->d_idx.as<uint32_t>(),
-                                                           nullptr);
-        ++launches;
+            pixelise_kernel<false, true><<<nb, threads, 0, st>>>(lon, lat, values, weights, nchan, n, rg, keys, rank,
+                                                                 nullptr, bins);
         HCG_CUDA(c, cudaGetLastError());
-    }
-    if (c->opt_profile) cudaEventRecord(c->ev[1], st);
-    if (n > 0) {
-        HCG_CUDA(c, cub::DeviceRadixSort::SortPairs(c->d_sort_tmp.p, tmp_bytes, c->d_keys.as<uint32_t>(),
-                                                    c->d_keys_out.as<uint32_t>(), c->d_idx.as<uint32_t>(),
-                                                    c->d_idx_out.as<uint32_t>(), n, 0, end_bit, st));
-        launches += 2 + (end_bit + 7) / 8;   // CUB onesweep: histogram + scan + one pass per digit
-    }
-    if (c->opt_profile) cudaEventRecord(c->ev[2], st);
-    {
-        // a4 (+ a5 in fp32 mode: the gather rides on the same pass over the sorted pairs)
-        const unsigned nb2 = (unsigned)((nn + 1 + threads - 1) / threads);
-        tables_pack_kernel<<<nb2, threads, 0, st>>>(c->d_keys_out.as<uint32_t>(), c->d_idx_out.as<uint32_t>(), n,
-                                                    (int32_t)rg.nbins, c->d_bins.as<int32_t>(),
-                                                    f32 && n > 0 ? c->d_misc.as<Rec32>() : nullptr,
-                                                    c->d_rec.as<Rec32>());
-        ++launches;
+        if (c->opt_profile) cudaEventRecord(c->ev[1], st);
+        HCG_CUDA(c, cub::DeviceScan::ExclusiveSum(c->d_sort_tmp.p, tmp_bytes, bins, bins, (int64_t)rg.nbins + 1, st));
+        scatter_index_kernel<<<nb, threads, 0, st>>>(keys, rank, n, (int32_t)rg.nbins, bins, sidx);
         HCG_CUDA(c, cudaGetLastError());
+        if (c->opt_profile) cudaEventRecord(c->ev[2], st);
+        const unsigned nbb = (unsigned)(((size_t)rg.nbins + threads - 1) / threads);
+        bin_order_kernel<<<nbb, threads, 0, st>>>((int32_t)rg.nbins, bins, sidx);
+        HCG_CUDA(c, cudaGetLastError());
+        launches = 5;                        // pixelise, scan (2 kernels), scatter, order
+        if (c->opt_profile) cudaEventRecord(c->ev[3], st);
+        if (f32) {
+            pack32_kernel<<<nb, threads, 0, st>>>(sidx, n, bins + rg.nbins, c->d_misc.as<Rec32>(), c->d_rec.as<Rec32>());
+            ++launches;
+            HCG_CUDA(c, cudaGetLastError());
+        }
+    } else {
+        if (n > 0) {
+            if (f32)
+                pixelise_kernel<true, false><<<nb, threads, 0, st>>>(lon, lat, values, weights, nchan, n, rg,
+                                                                     c->d_keys.as<uint32_t>(), c->d_idx.as<uint32_t>(),
+                                                                     c->d_misc.as<Rec32>(), nullptr);
+            else
+                pixelise_kernel<false, false><<<nb, threads, 0, st>>>(lon, lat, values, weights, nchan, n, rg,
+                                                                      c->d_keys.as<uint32_t>(), c->d_idx.as<uint32_t>(),
+                                                                      nullptr, nullptr);
+            ++launches;
+            HCG_CUDA(c, cudaGetLastError());
+        }
+        if (c->opt_profile) cudaEventRecord(c->ev[1], st);
+        if (n > 0) {
+            HCG_CUDA(c, cub::DeviceRadixSort::SortPairs(c->d_sort_tmp.p, tmp_bytes, c->d_keys.as<uint32_t>(),
+                                                        c->d_keys_out.as<uint32_t>(), c->d_idx.as<uint32_t>(),
+                                                        c->d_idx_out.as<uint32_t>(), n, 0, end_bit, st));
+            launches += 2 + (end_bit + 7) / 8;   // CUB onesweep: histogram + scan + one pass per digit
+        }
+        if (c->opt_profile) cudaEventRecord(c->ev[2], st);
+        {
+            // a4 (+ a5 in fp32 mode: the gather rides on the same pass over the sorted pairs)
+            const unsigned nb2 = (unsigned)((nn + 1 + threads - 1) / threads);
+            tables_pack_kernel<<<nb2, threads, 0, st>>>(c->d_keys_out.as<uint32_t>(), c->d_idx_out.as<uint32_t>(), n,
+                                                        (int32_t)rg.nbins, c->d_bins.as<int32_t>(),
+                                                        f32 && n > 0 ? c->d_misc.as<Rec32>() : nullptr,
+                                                        c->d_rec.as<Rec32>());
+            ++launches;
+            HCG_CUDA(c, cudaGetLastError());
+        }
+        if (c->opt_profile) cudaEventRecord(c->ev[3], st);
     }
-    if (c->opt_profile) cudaEventRecord(c->ev[3], st);
     if (n > 0 && !f32) {
-        pack64_kernel<<<nb, threads, 0, st>>>(c->d_keys_out.as<uint32_t>(), c->d_idx_out.as<uint32_t>(), n,
-                                              (uint32_t)rg.nbins, lon, lat, weights, c->d_rec.as<Rec64>());
+        pack64_kernel<<<nb, threads, 0, st>>>(c->d_idx_out.as<uint32_t>(), n, c->d_bins.as<int32_t>() + rg.nbins, lon,
+                                              lat, weights, c->d_rec.as<Rec64>());
         ++launches;
         HCG_CUDA(c, cudaGetLastError());
     }

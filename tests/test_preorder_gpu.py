@@ -89,3 +89,74 @@ def test_measured_peaks_are_plausible():
     from paper_2012_13173_b200 import binding
     fp32, mufu = binding.measure_peaks(0)
     assert 5e12 < fp32 < 6e13 and 5e11 < mufu < 8e12
+
+
+def _run_preorder_mode(w, mode, precision="f32", lon=None, lat=None, values=None, weights=None):
+    from paper_2012_13173_b200 import binding
+    g = binding.HCGrid(w.sigma_deg, w.radius_deg, w.nside, precision=precision)
+    t = w.target
+    g.set_target_car(t.nx, t.ny, t.lon0, t.lat0, t.dlon, t.dlat)
+    g.set_option(binding.OPT_PREORDER, mode)
+    lon = w.lon if lon is None else lon
+    lat = w.lat if lat is None else lat
+    values = w.values if values is None else values
+    cube, wmap, cnt = g.grid(_dev(lon), _dev(lat), _dev(values), None if weights is None else _dev(weights))
+    torch.cuda.synchronize()
+    pre = g.debug_preorder()
+    st = g.stats()
+    g.close()
+    return cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy(), pre, st
+
+
+@pytest.mark.parametrize("case", ["c1", "c3", "c4", "c3_f64", "pileup", "pileup_f64", "weights"])
+def test_counting_preorder_gives_the_radix_sort_order(case):
+    """The counting pre-order (atomics + scan + per-bin index sort) must reproduce the stable
+    key-value sort of PAPER.md:120 exactly: same S' (sorted indices), same tables, and hence
+    bit-identical maps."""
+    from paper_2012_13173_b200 import binding
+    precision = "f64" if case.endswith("f64") else "f32"
+    kw = {}
+    if case == "c1":
+        w = workloads.make(1, 1.0)
+    elif case == "c4":
+        w = workloads.make(4, 0.01)
+    else:
+        w = workloads.make(3, 0.004)
+    if case.startswith("pileup"):
+        # a third of the samples stare at three points: bins of thousands of samples next to
+        # sparse ones (the block-sorted path), plus exact duplicates
+        rng = np.random.default_rng(77)
+        lon, lat = w.lon.copy(), w.lat.copy()
+        t = w.target
+        n = lon.size
+        for k, frac in enumerate((0.2, 0.1, 0.03)):
+            sel = rng.choice(n, int(frac * n), replace=False)
+            lon[sel] = t.lon0 + (0.3 + 0.2 * k) * t.nx * t.dlon + rng.normal(0, 1e-7, sel.size) * (k != 2)
+            lat[sel] = t.lat0 + (0.4 + 0.1 * k) * t.ny * t.dlat + rng.normal(0, 1e-7, sel.size) * (k != 2)
+        kw = {"lon": lon, "lat": lat}
+    if case == "weights":
+        kw = {"weights": np.random.default_rng(3).uniform(0.5, 2.0, w.n).astype(np.float32)}
+    a = _run_preorder_mode(w, binding.PREORDER_RADIX, precision, **kw)
+    b = _run_preorder_mode(w, binding.PREORDER_COUNTING, precision, **kw)
+    assert a[4]["preorder"] == 1 and b[4]["preorder"] == 2
+    assert a[4]["n_kept"] == b[4]["n_kept"] > 0
+    assert np.array_equal(a[3][1], b[3][1])                   # sorted indices: the same S'
+    assert np.array_equal(a[3][0], b[3][0]) and np.array_equal(a[3][3], b[3][3])
+    assert np.array_equal(a[2], b[2])
+    assert np.array_equal(a[1], b[1])
+    assert np.array_equal(a[0], b[0], equal_nan=True)
+
+
+def test_preorder_auto_choice():
+    """Auto: counting unless samples outnumber bins many times over (or bins the samples)."""
+    from paper_2012_13173_b200 import binding
+    w = workloads.make(3, 0.004)
+    st = _run_preorder_mode(w, binding.PREORDER_AUTO)[4]
+    assert st["preorder"] == 2
+    # the same field with 20 x the samples piled on: far more samples than bins
+    rng = np.random.default_rng(1)
+    lon = np.tile(w.lon, 40) + rng.normal(0, 1e-4, w.n * 40)
+    lat = np.tile(w.lat, 40)
+    val = np.tile(w.values, (40, 1))
+    st2 = _run_preorder_mode(w, binding.PREORDER_AUTO, lon=lon, lat=lat, values=val)[4]
+    assert st2["preorder"] == (2 if lon.size <= 4 * st2["n_bins"] else 1)
