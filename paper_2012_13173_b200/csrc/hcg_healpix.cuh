@@ -87,27 +87,28 @@ HCG_HD void ang2ring(int nside, double lon, double lat, int& iring, int& ip) {
     if (za <= 2.0 / 3.0) {                         // equatorial belt
         const double t1 = n * (0.5 + tt);
         const double t2 = n * z * 0.75;
-        const long long jp = (long long)floor(t1 - t2);   // ascending edge line index
-        const long long jm = (long long)floor(t1 + t2);   // descending edge line index
-        const long long ir = nside + 1 + jp - jm;         // in {1, 2n+1}
-        const long long kshift = 1 - (ir & 1);
-        long long p = (jp + jm - nside + kshift + 1) >> 1;
-        p %= 4LL * nside;
-        if (p < 0) p += 4LL * nside;
-        iring = (int)(ir + nside - 1);
-        ip = (int)p;
+        // all of these are below 6 nside <= 49152 in magnitude: 32-bit integers throughout
+        const int jp = (int)floor(t1 - t2);               // ascending edge line index
+        const int jm = (int)floor(t1 + t2);               // descending edge line index
+        const int ir = nside + 1 + jp - jm;               // in {1, 2n+1}
+        const int kshift = 1 - (ir & 1);
+        int p = (jp + jm - nside + kshift + 1) >> 1;      // in (-nside, 5 nside]
+        if (p >= 4 * nside) p -= 4 * nside;
+        if (p < 0) p += 4 * nside;
+        iring = ir + nside - 1;
+        ip = p;
     } else {                                       // polar caps
         const double tp = tt - floor(tt);
         const double sh = sin(0.5 * (kHalfPi - fabs(lat)));
         const double tmp = n * kSqrt6 * sh;     // n sqrt(3 (1 - |z|)), 1-|z| = 2 sin^2(colat/2)
-        long long jp = (long long)(tp * tmp);
-        long long jm = (long long)((1.0 - tp) * tmp);
-        long long ir = jp + jm + 1;                // ring counted from the closest pole
+        const int jp = (int)(tp * tmp);
+        const int jm = (int)((1.0 - tp) * tmp);
+        int ir = jp + jm + 1;                      // ring counted from the closest pole
         if (ir > nside) ir = nside;
-        long long p = (long long)(tt * (double)ir);
-        p %= 4 * ir;
-        iring = (int)(z > 0 ? ir : 4LL * nside - ir);
-        ip = (int)p;
+        int p = (int)(tt * (double)ir);            // tt in [0, 4): p in [0, 4 ir]
+        if (p >= 4 * ir) p -= 4 * ir;
+        iring = z > 0 ? ir : 4 * nside - ir;
+        ip = p;
     }
 }
 
@@ -121,16 +122,16 @@ HCG_HD long long ring_bin(int iring, int nside, int ip, double lon, int b) {
     double d = g - (double)ip;
     if (d > 0.5 * npr) d -= npr;
     if (d < -0.5 * npr) d += npr;
-    long long sub = (long long)floor(d * (double)(1 << b));
+    int sub = (int)floor(d * (double)(1 << b));
     if (sub < 0) sub = 0;
     if (sub > (1 << b) - 1) sub = (1 << b) - 1;
-    return ((long long)ip << b) + sub;
+    return (long long)((ip << b) + sub);           // < 4 nside 2^b <= 2^21
 }
 
 // number of lookup bins along ring `iring`
 HCG_HD long long ring_nbins(int iring, int nside, int b) {
-    const long long npr = ring_npix(iring, nside);
-    return b >= 0 ? (npr << b) : (((npr - 1) >> (-b)) + 1);
+    const int npr = ring_npix(iring, nside);
+    return (long long)(b >= 0 ? (npr << b) : (((npr - 1) >> (-b)) + 1));
 }
 
 // bin coordinate (real) of longitude lon on ring iring: floor() of it is the bin of a
@@ -138,7 +139,8 @@ HCG_HD long long ring_nbins(int iring, int nside, int b) {
 HCG_HD double ring_bin_coord(int iring, int nside, double lon, int b) {
     const int npr = ring_npix(iring, nside);
     const double g = lon * ((double)npr * kInvTwoPi) + ring_off(iring, nside);
-    return ldexp(g, b);
+    // g * 2^b, exact (the value ldexp(g, b) returns); |b| < 16
+    return b >= 0 ? g * (double)(1 << b) : g * (1.0 / (double)(1 << (-b)));
 }
 
 }  // namespace hcg

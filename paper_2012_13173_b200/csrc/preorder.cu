@@ -178,10 +178,24 @@ bin_order_kernel(int32_t nbins, const int32_t* __restrict__ bin_start, uint32_t*
         if (cnt > kThreadSortMax) {
             const int slot = atomicAdd(&s_cnt, 1);
             s_lo[slot] = s; s_len[slot] = cnt;
-        } else if (cnt == 2) {
-            const uint32_t x = sidx[s], y = sidx[s + 1];
-            if (x > y) { sidx[s] = y; sidx[s + 1] = x; }
-        } else if (cnt > 2) {
+        } else if (cnt >= 2 && cnt <= 8) {
+            // up to 8: registers and a fixed 19-comparator network (Batcher's merge exchange),
+            // one memory round trip whatever the count; the padding sorts to the top
+            uint32_t v[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) v[k] = k < cnt ? sidx[s + k] : 0xffffffffu;
+#define HCG_CX(i, j) { const uint32_t lo_ = min(v[i], v[j]), hi_ = max(v[i], v[j]); v[i] = lo_; v[j] = hi_; }
+            HCG_CX(0, 1) HCG_CX(2, 3) HCG_CX(4, 5) HCG_CX(6, 7)
+            HCG_CX(0, 2) HCG_CX(1, 3) HCG_CX(4, 6) HCG_CX(5, 7)
+            HCG_CX(1, 2) HCG_CX(5, 6)
+            HCG_CX(0, 4) HCG_CX(1, 5) HCG_CX(2, 6) HCG_CX(3, 7)
+            HCG_CX(2, 4) HCG_CX(3, 5)
+            HCG_CX(1, 2) HCG_CX(3, 4) HCG_CX(5, 6)
+#undef HCG_CX
+#pragma unroll
+            for (int k = 0; k < 8; ++k)
+                if (k < cnt) sidx[s + k] = v[k];
+        } else if (cnt > 8) {
             for (int a = s + 1; a < e; ++a) {               // insertion sort, in place
                 const uint32_t v = sidx[a];
                 int p = a;
