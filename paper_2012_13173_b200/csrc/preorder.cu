@@ -159,7 +159,7 @@ __device__ void block_sort_u32(uint32_t* a, int L, int tid, int nthr) {
     }
 }
 
-constexpr int kThreadSortMax = 12;   // longer bins are sorted by the whole block
+constexpr int kThreadSortMax = 32;   // longer bins are sorted by the whole block
 
 // Thread b owns bin b: orders sidx[bin_start[b], bin_start[b+1]) ascending.  Bins longer than
 // kThreadSortMax are queued in shared memory and sorted by the whole block (rare unless
@@ -243,9 +243,13 @@ int run_preorder(hcgrid_ctx* c, int64_t n, const double* lon, const double* lat,
                  int nchan, const float* weights, cudaStream_t st) {
     const Region& rg = c->region;
     const bool f32 = c->precision == HCGRID_F32 && c->f32_series_ok && c->opt_kernel != 2;
-    // counting pre-order unless the samples pile up (long bins, contended counters) or the
-    // option says otherwise; the result is the same S' either way
-    const bool counting = n > 0 && (c->opt_preorder == 2 || (c->opt_preorder == 0 && n <= 4 * (int64_t)rg.nbins && (int64_t)rg.nbins <= 16 * n));
+    // counting pre-order unless the samples pile up (long bins to order), the table is far
+    // larger than the input (its O(bins) passes), or the option says otherwise; the result is
+    // the same S' either way
+    const int64_t nbins64 = (int64_t)rg.nbins;
+    const bool counting = n > 0 && (c->opt_preorder == 2 ||
+                                    (c->opt_preorder == 0 && n <= 4 * nbins64 &&
+                                     (nbins64 <= 16 * n || nbins64 <= ((int64_t)1 << 22))));
     const size_t nn = (size_t)(n > 0 ? n : 1);
     HCG_CUDA(c, c->d_keys.ensure(nn * 4));
     HCG_CUDA(c, c->d_idx.ensure(nn * 4));
