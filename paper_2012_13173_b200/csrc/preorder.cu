@@ -159,11 +159,10 @@ __device__ void block_sort_u32(uint32_t* a, int L, int tid, int nthr) {
     }
 }
 
-constexpr int kThreadSortMax = 32;   // longer bins are sorted by the whole block
+constexpr int kInsertReach = 48;     // positions an index may travel in the thread-serial pass
 
-// Thread b owns bin b: orders sidx[bin_start[b], bin_start[b+1]) ascending.  Bins longer than
-// kThreadSortMax are queued in shared memory and sorted by the whole block (rare unless
-// samples pile up in one place).
+// Thread b owns bin b: orders sidx[bin_start[b], bin_start[b+1]) ascending.  Bins the thread
+// cannot finish (see below) are queued in shared memory and sorted by the whole block.
 __global__ void __launch_bounds__(256)
 bin_order_kernel(int32_t nbins, const int32_t* __restrict__ bin_start, uint32_t* sidx) {
     __shared__ int s_cnt;
@@ -175,9 +174,31 @@ bin_order_kernel(int32_t nbins, const int32_t* __restrict__ bin_start, uint32_t*
     if (b < nbins) {
         const int s = bin_start[b], e = bin_start[b + 1];
         const int cnt = e - s;
-        if (cnt > kThreadSortMax) {
-            const int slot = atomicAdd(&s_cnt, 1);
-            s_lo[slot] = s; s_len[slot] = cnt;
+        if (cnt > 8) {
+            // Arrival order follows launch order up to the samples in flight together, so a
+            // long bin is ascending but for short-range disorder: one insertion pass with the
+            // running maximum in a register and a bounded reach.  Whoever needs to travel
+            // further than kInsertReach sends the bin to the block sort below.
+            bool far = false;
+            uint32_t top = sidx[s];
+            for (int a = s + 1; a < e; ++a) {
+                const uint32_t v = sidx[a];
+                if (v >= top) { top = v; continue; }
+                int p = a;
+                const int stop = max(s, a - kInsertReach);
+                while (p > stop) {
+                    const uint32_t u = sidx[p - 1];
+                    if (u <= v) break;
+                    sidx[p] = u;
+                    --p;
+                }
+                sidx[p] = v;
+                far |= p == stop && p > s && sidx[p - 1] > v;
+            }
+            if (far) {
+                const int slot = atomicAdd(&s_cnt, 1);
+                s_lo[slot] = s; s_len[slot] = cnt;
+            }
         } else if (cnt >= 2 && cnt <= 8) {
             // up to 8: registers and a fixed 19-comparator network (Batcher's merge exchange),
             // one memory round trip whatever the count; the padding sorts to the top
@@ -195,18 +216,6 @@ bin_order_kernel(int32_t nbins, const int32_t* __restrict__ bin_start, uint32_t*
 #pragma unroll
             for (int k = 0; k < 8; ++k)
                 if (k < cnt) sidx[s + k] = v[k];
-        } else if (cnt > 8) {
-            for (int a = s + 1; a < e; ++a) {               // insertion sort, in place
-                const uint32_t v = sidx[a];
-                int p = a;
-                while (p > s) {
-                    const uint32_t u = sidx[p - 1];
-                    if (u <= v) break;
-                    sidx[p] = u;
-                    --p;
-                }
-                sidx[p] = v;
-            }
         }
     }
     __syncthreads();
@@ -248,7 +257,7 @@ int run_preorder(hcgrid_ctx* c, int64_t n, const double* lon, const double* lat,
     // the same S' either way
     const int64_t nbins64 = (int64_t)rg.nbins;
     const bool counting = n > 0 && (c->opt_preorder == 2 ||
-                                    (c->opt_preorder == 0 && n <= 4 * nbins64 &&
+                                    (c->opt_preorder == 0 && n <= 16 * nbins64 &&
                                      (nbins64 <= 16 * n || nbins64 <= ((int64_t)1 << 22))));
     const size_t nn = (size_t)(n > 0 ? n : 1);
     HCG_CUDA(c, c->d_keys.ensure(nn * 4));

@@ -153,10 +153,10 @@ def test_preorder_auto_choice():
     w = workloads.make(3, 0.004)
     st = _run_preorder_mode(w, binding.PREORDER_AUTO)[4]
     assert st["preorder"] == 2
-    # the same field with 20 x the samples piled on: far more samples than bins
+    # the same field with 40 x the samples piled on: far more samples than bins
     rng = np.random.default_rng(1)
     lon = np.tile(w.lon, 40) + rng.normal(0, 1e-4, w.n * 40)
     lat = np.tile(w.lat, 40)
     val = np.tile(w.values, (40, 1))
     st2 = _run_preorder_mode(w, binding.PREORDER_AUTO, lon=lon, lat=lat, values=val)[4]
-    assert st2["preorder"] == (2 if lon.size <= 4 * st2["n_bins"] else 1)
+    assert st2["preorder"] == (2 if lon.size <= 16 * st2["n_bins"] else 1)
