@@ -39,12 +39,27 @@ double hcgrid_oracle_distance(double lon1_deg, double lat1_deg,
 
 int hcgrid_oracle_last_threads(void) { return g_last_threads; }
 
-int hcgrid_oracle_grid(double sigma_deg, double radius_deg,
-                       int64_t ncell, const double* cell_lon, const double* cell_lat,
-                       int64_t n, const double* lon, const double* lat,
-                       const float* values, int32_t nchan, const float* weights,
-                       double* datacube, double* weightmap, int64_t* counts,
-                       double* absmap, int64_t* near_boundary, int nthreads)
+/* Kernel weight as a function of the great-circle angle d (rad).
+ *   ktype 0: Gaussian exp(-d^2 / (2 sigma^2))                       (the default)
+ *   ktype 1: tapered sinc  sinc(d / (b sigma)) exp(-(d / (a sigma))^2),  sinc(x) = sin(pi x)/(pi x)
+ *            -- the finite-length stand-in for the "sinc function with infinite length" of
+ *            PAPER.md:186, in the form of the work the paper follows for its kernel set-up
+ *            (Winkel et al. 2016b); may be negative. */
+static double kernel_weight(int ktype, double d, double sigma, double ka, double kb)
+{
+    if (ktype == 0) return exp(-d * d / (2.0 * sigma * sigma));
+    const double x = d / sigma;
+    const double y = 3.14159265358979323846 * x / kb;
+    const double sinc = y == 0.0 ? 1.0 : sin(y) / y;
+    return sinc * exp(-(x / ka) * (x / ka));
+}
+
+static int grid_core(int ktype, double ka, double kb, double sigma_deg, double radius_deg,
+                     int64_t ncell, const double* cell_lon, const double* cell_lat,
+                     int64_t n, const double* lon, const double* lat,
+                     const float* values, int32_t nchan, const float* weights,
+                     double* datacube, double* weightmap, int64_t* counts,
+                     double* absmap, double* abswmap, int64_t* near_boundary, int nthreads)
 {
     if (!(sigma_deg > 0.0) || !(radius_deg > 0.0) || ncell < 0 || n < 0 || nchan < 1)
         return -1;
@@ -78,7 +93,7 @@ int hcgrid_oracle_grid(double sigma_deg, double radius_deg,
 #pragma omp for schedule(dynamic, 16)
         for (int64_t c = 0; c < ncell; ++c) {
             if (!S || !A) continue;
-            long double W = 0.0L;
+            long double W = 0.0L, Wabs = 0.0L;
             int64_t cnt = 0, nb = 0;
             for (int k = 0; k < nchan; ++k) { S[k] = 0.0L; A[k] = 0.0L; }
             const double clon = cell_lon[c], clat = cell_lat[c];
@@ -87,27 +102,32 @@ int hcgrid_oracle_grid(double sigma_deg, double radius_deg,
                 const double d = hcgrid_oracle_distance(clon, clat, lon[s], lat[s]);
                 if (fabs(d - R) < 1e-9) nb++;
                 if (d <= R) {
-                    const double w = exp(-d * d * inv2s2);
+                    const double w = ktype == 0 ? exp(-d * d * inv2s2) : kernel_weight(ktype, d, sigma, ka, kb);
                     const double q = weights ? (double)weights[s] : 1.0;
                     const double qw = q * w;
                     W += (long double)qw;
+                    Wabs += (long double)fabs(qw);
                     cnt++;
                     const float* v = values + (size_t)s * (size_t)nchan;
                     for (int k = 0; k < nchan; ++k) {
                         const double vk = (double)v[k];
                         S[k] += (long double)(qw * vk);
-                        A[k] += (long double)(qw * fabs(vk));
+                        A[k] += (long double)(fabs(qw) * fabs(vk));
                     }
                 }
             }
             weightmap[c] = (double)W;
+            if (abswmap) abswmap[c] = (double)Wabs;
             if (counts) counts[c] = cnt;
             if (near_boundary) near_boundary[c] = nb;
+            /* Gaussian: W > 0 as soon as one sample contributes.  Signed kernels: W != 0. */
+            const int defined = ktype == 0 ? (W > 0.0L) : (W != 0.0L);
             for (int k = 0; k < nchan; ++k) {
                 size_t o = (size_t)c * (size_t)nchan + (size_t)k;
-                if (W > 0.0L) {
+                if (defined) {
                     datacube[o] = (double)(S[k] / W);
-                    if (absmap) absmap[o] = (double)(A[k] / W);
+                    /* tolerance scale: sum |q w| |v| over |W| (equals sum q w |v| / W for w >= 0) */
+                    if (absmap) absmap[o] = (double)(A[k] / fabsl(W));
                 } else {
                     datacube[o] = NAN;
                     if (absmap) absmap[o] = NAN;
@@ -118,4 +138,28 @@ int hcgrid_oracle_grid(double sigma_deg, double radius_deg,
         free(A);
     }
     return failed ? -1 : 0;
+}
+
+int hcgrid_oracle_grid(double sigma_deg, double radius_deg,
+                       int64_t ncell, const double* cell_lon, const double* cell_lat,
+                       int64_t n, const double* lon, const double* lat,
+                       const float* values, int32_t nchan, const float* weights,
+                       double* datacube, double* weightmap, int64_t* counts,
+                       double* absmap, int64_t* near_boundary, int nthreads)
+{
+    return grid_core(0, 0.0, 0.0, sigma_deg, radius_deg, ncell, cell_lon, cell_lat, n, lon, lat, values, nchan,
+                     weights, datacube, weightmap, counts, absmap, NULL, near_boundary, nthreads);
+}
+
+int hcgrid_oracle_grid_kernel(int ktype, double ka, double kb, double sigma_deg, double radius_deg,
+                              int64_t ncell, const double* cell_lon, const double* cell_lat,
+                              int64_t n, const double* lon, const double* lat,
+                              const float* values, int32_t nchan, const float* weights,
+                              double* datacube, double* weightmap, int64_t* counts,
+                              double* absmap, double* abswmap, int64_t* near_boundary, int nthreads)
+{
+    if (ktype != 0 && ktype != 1) return -1;
+    if (ktype == 1 && (!(ka > 0.0) || !(kb > 0.0))) return -1;
+    return grid_core(ktype, ka, kb, sigma_deg, radius_deg, ncell, cell_lon, cell_lat, n, lon, lat, values, nchan,
+                     weights, datacube, weightmap, counts, absmap, abswmap, near_boundary, nthreads);
 }

@@ -61,6 +61,21 @@ int hcgrid_oracle_grid(double sigma_deg, double radius_deg,
                        double* datacube, double* weightmap, int64_t* counts,
                        double* absmap, int64_t* near_boundary, int nthreads);
 
+/* The same loop with the kernel function chosen by ktype:
+ *   0  Gaussian exp(-d^2 / (2 sigma^2)) (ka, kb ignored) -- identical to hcgrid_oracle_grid;
+ *   1  tapered sinc: sinc(d / (kb sigma)) * exp(-(d / (ka sigma))^2), sinc(x) = sin(pi x) / (pi x)
+ *      (PAPER.md:186 names the sinc as the optimal kernel and finite-length functions as what
+ *      is used in practice; the tapered form is that of the work it follows, Winkel et al. 2016b).
+ * Signed weights change two outputs: datacube = S / W wherever W != 0 (NaN otherwise), and
+ * absmap = sum |q w| |v| / |W|.  abswmap[ncell] (may be NULL) = sum |q w|, the scale against
+ * which W itself is to be compared (W can cancel to ~0).  Returns 0, or -1 on invalid arguments. */
+int hcgrid_oracle_grid_kernel(int ktype, double ka, double kb, double sigma_deg, double radius_deg,
+                              int64_t ncell, const double* cell_lon, const double* cell_lat,
+                              int64_t n, const double* lon, const double* lat,
+                              const float* values, int32_t nchan, const float* weights,
+                              double* datacube, double* weightmap, int64_t* counts,
+                              double* absmap, double* abswmap, int64_t* near_boundary, int nthreads);
+
 /* Number of OpenMP threads the last hcgrid_oracle_grid call used. */
 int hcgrid_oracle_last_threads(void);
 

@@ -43,6 +43,9 @@ def _load():
         lib.hcgrid_oracle_grid.restype = ctypes.c_int
         lib.hcgrid_oracle_grid.argtypes = [d, d, ctypes.c_int64, p, p, ctypes.c_int64, p, p, p,
                                            ctypes.c_int32, p, p, p, p, p, p, ctypes.c_int]
+        lib.hcgrid_oracle_grid_kernel.restype = ctypes.c_int
+        lib.hcgrid_oracle_grid_kernel.argtypes = [ctypes.c_int, d, d, d, d, ctypes.c_int64, p, p, ctypes.c_int64, p, p,
+                                                  p, ctypes.c_int32, p, p, p, p, p, p, p, ctypes.c_int]
         lib.hcgrid_oracle_last_threads.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -62,15 +65,20 @@ class OracleResult:
     absmap: np.ndarray         # [ncell, nchan] float64: sum q w |v| / W
     near_boundary: np.ndarray  # [ncell] int64: pairs with |d - R| < 1e-9 rad
     threads: int
+    abswmap: np.ndarray = None  # [ncell] float64: sum |q w| (kernel= calls only)
 
 
 def _ptr(a):
     return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
 
 
+GAUSS, TAPERED_SINC = 0, 1
+
+
 def grid(sigma_deg, radius_deg, cell_lon, cell_lat, lon, lat, values, weights=None,
-         nthreads: int = 0) -> OracleResult:
-    """Brute-force Eq. 1 over every (cell, sample) pair.  Angles in degrees."""
+         nthreads: int = 0, kernel=None) -> OracleResult:
+    """Brute-force Eq. 1 over every (cell, sample) pair.  Angles in degrees.
+    kernel = None (Gaussian, hcgrid_oracle_grid) or (ktype, ka, kb) (hcgrid_oracle_grid_kernel)."""
     lib = _load()
     cell_lon = np.ascontiguousarray(cell_lon, dtype=np.float64).ravel()
     cell_lat = np.ascontiguousarray(cell_lat, dtype=np.float64).ravel()
@@ -95,6 +103,16 @@ def grid(sigma_deg, radius_deg, cell_lon, cell_lat, lon, lat, values, weights=No
     counts = np.empty(ncell, dtype=np.int64)
     absmap = np.empty((ncell, nchan), dtype=np.float64)
     nb = np.empty(ncell, dtype=np.int64)
+    if kernel is not None:
+        ktype, ka, kb = kernel
+        absw = np.empty(ncell, dtype=np.float64)
+        rc = lib.hcgrid_oracle_grid_kernel(int(ktype), float(ka), float(kb), float(sigma_deg), float(radius_deg),
+                                           ncell, _ptr(cell_lon), _ptr(cell_lat), n, _ptr(lon), _ptr(lat),
+                                           _ptr(values), nchan, _ptr(weights), _ptr(cube), _ptr(wmap),
+                                           _ptr(counts), _ptr(absmap), _ptr(absw), _ptr(nb), int(nthreads))
+        if rc != 0:
+            raise ValueError("hcgrid_oracle_grid_kernel rejected its arguments")
+        return OracleResult(cube, wmap, counts, absmap, nb, int(lib.hcgrid_oracle_last_threads()), absw)
     rc = lib.hcgrid_oracle_grid(float(sigma_deg), float(radius_deg), ncell, _ptr(cell_lon),
                                 _ptr(cell_lat), n, _ptr(lon), _ptr(lat), _ptr(values), nchan,
                                 _ptr(weights), _ptr(cube), _ptr(wmap), _ptr(counts),

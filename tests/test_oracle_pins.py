@@ -254,3 +254,65 @@ def test_batches_are_additive_in_the_unnormalised_sums(oracle):
     np.testing.assert_allclose(w, full.weightmap, rtol=1e-13)
     np.testing.assert_allclose(v, full.datacube, rtol=1e-11, atol=1e-13, equal_nan=True)
     assert (full.weightmap == 0).any() and (full.weightmap > 0).any()      # the case has empty cells too
+
+
+# ---------------------------------------------------------------- tapered-sinc kernel (S:8f NEXT-3)
+def test_tapered_sinc_zeros_sign_and_special_points(oracle):
+    """One sample on the cells' meridian, so d is a latitude difference exactly.  sinc(d/(b sigma)) has
+    its zeros at d = k b sigma, is 1 at d = 0 and -2/(3 pi) at d = 1.5 b sigma (sin(3 pi/2) = -1);
+    catches: a missing pi, a and b swapped, sigma^2 against sigma, a Gaussian taper with the
+    factor 1/2 left in."""
+    sigma, a, b = 0.1, 2.52, 1.55
+    d_deg = np.array([0.0, b * sigma, 2 * b * sigma, 1.5 * b * sigma, 0.5 * b * sigma])
+    res = oracle.grid(sigma, 5 * sigma, np.full(5, 40.0), 10.0 + d_deg, [40.0], [10.0], [2.0],
+                      kernel=(oracle.TAPERED_SINC, a, b))
+    w = res.weightmap
+    assert w[0] == 1.0
+    assert abs(w[1]) < 1e-12 and abs(w[2]) < 1e-12                      # zeros of the sinc
+    assert w[3] == pytest.approx(-2.0 / (3.0 * math.pi) * math.exp(-(1.5 * b / a) ** 2), rel=1e-12)
+    assert w[4] == pytest.approx(2.0 / math.pi * math.exp(-(0.5 * b / a) ** 2), rel=1e-12)   # sin(pi/2) = 1
+    assert np.all(res.counts == 1)
+    assert np.allclose(res.datacube[[0, 3, 4], 0], 2.0, rtol=1e-12)     # one sample: V = v whatever the sign of w
+    assert np.allclose(res.abswmap, np.abs(w), rtol=0, atol=1e-18)
+
+
+def test_tapered_sinc_reduces_to_the_gaussian(oracle):
+    """b -> infinity switches the sinc off; what is left, exp(-(d/(a sigma))^2), is the Gaussian of
+    width a sigma / sqrt 2 -- the routine pinned above.  Catches: taper exponent, any change to the
+    distance or the accumulation on the kernel path."""
+    rng = np.random.default_rng(5)
+    n = 400
+    lon = 100.0 + rng.uniform(-0.5, 0.5, n)
+    lat = -30.0 + rng.uniform(-0.5, 0.5, n)
+    val = rng.normal(size=(n, 3)).astype(np.float32)
+    wts = rng.uniform(0.5, 2.0, n).astype(np.float32)
+    clon, clat = np.meshgrid(100.0 + np.linspace(-0.4, 0.4, 7), -30.0 + np.linspace(-0.4, 0.4, 7))
+    sigma, a = 0.05, 2.52
+    k = oracle.grid(sigma, 0.2, clon, clat, lon, lat, val, wts, kernel=(oracle.TAPERED_SINC, a, 1e12))
+    g = oracle.grid(a * sigma / math.sqrt(2.0), 0.2, clon, clat, lon, lat, val, wts)
+    assert np.array_equal(k.counts, g.counts)
+    assert np.allclose(k.weightmap, g.weightmap, rtol=1e-12)
+    assert np.allclose(k.datacube, g.datacube, rtol=1e-11, atol=1e-13, equal_nan=True)
+    # and ktype 0 through the kernel entry IS the Gaussian entry
+    k0 = oracle.grid(sigma, 0.2, clon, clat, lon, lat, val, wts, kernel=(oracle.GAUSS, 0.0, 0.0))
+    g0 = oracle.grid(sigma, 0.2, clon, clat, lon, lat, val, wts)
+    assert np.array_equal(k0.weightmap, g0.weightmap) and np.array_equal(k0.datacube, g0.datacube, equal_nan=True)
+
+
+def test_tapered_sinc_constant_field_and_negative_lobes(oracle):
+    """Eq. 1 normalises by W, so a constant field grids to the constant wherever W != 0 even
+    with negative weights; with R = 3 sigma (> b sigma) some pairs do sit in the negative lobe."""
+    rng = np.random.default_rng(6)
+    n = 3000
+    lon = 10.0 + rng.uniform(-1, 1, n)
+    lat = 50.0 + rng.uniform(-1, 1, n)
+    clon, clat = np.meshgrid(10.0 + np.linspace(-0.8, 0.8, 9), 50.0 + np.linspace(-0.8, 0.8, 9))
+    res = oracle.grid(0.1, 0.3, clon, clat, lon, lat, np.full(n, 3.25, np.float32),
+                      kernel=(oracle.TAPERED_SINC, 2.52, 1.55))
+    assert np.all(res.counts > 0)
+    assert np.all(res.abswmap > np.abs(res.weightmap) * (1 + 1e-9))     # negative contributions exist
+    assert np.allclose(res.datacube[:, 0], 3.25, rtol=1e-10)
+    with pytest.raises(ValueError):
+        oracle.grid(0.1, 0.3, [0.0], [0.0], [0.0], [0.0], [1.0], kernel=(1, 2.52, 0.0))
+    with pytest.raises(ValueError):
+        oracle.grid(0.1, 0.3, [0.0], [0.0], [0.0], [0.0], [1.0], kernel=(7, 1.0, 1.0))
