@@ -99,6 +99,22 @@ int hcgrid_destroy(hcgrid_ctx* ctx);
 
 int hcgrid_set_option(hcgrid_ctx* ctx, int option, int64_t value);
 
+/* Kernel function omega(d) of Eq. 1, d = great-circle angle, sigma and the
+ * support radius as given to hcgrid_create:
+ *   HCGRID_KERNEL_GAUSS         exp(-d^2 / (2 sigma^2)) -- the paper's kernel and the default; a, b ignored.
+ *   HCGRID_KERNEL_TAPERED_SINC  sinc(d / (b sigma)) exp(-(d / (a sigma))^2), sinc(x) = sin(pi x) / (pi x):
+ *                               the finite stand-in for the sinc PAPER.md:186 calls optimal, in the form of
+ *                               the work the paper follows there (Winkel et al. 2016b, who advise a = 2.52,
+ *                               b = 1.55; the caller's choice here).  Weights can
+ *                               be negative: the datacube is S / W wherever W != 0 (NaN otherwise) and the
+ *                               weight map may cancel towards zero.
+ * Takes effect at the next hcgrid_grid / hcgrid_accumulate; not allowed while an accumulation is open.
+ * Gaussian runs on every convolution kernel; other functions on the general kernels only
+ * (any target, any channel count, both precisions).  Returns HCGRID_ERR_INVALID_ARG for an
+ * unknown type or non-positive a, b. */
+enum { HCGRID_KERNEL_GAUSS = 0, HCGRID_KERNEL_TAPERED_SINC = 1 };
+int hcgrid_set_kernel(hcgrid_ctx* ctx, int32_t kernel_type, double a, double b);
+
 /* Target = plate-carree grid: cell (ix, iy) centre = (lon0 + ix*dlon, lat0 + iy*dlat),
  * each evaluated with one rounding per operation (no FMA); dlon, dlat may be negative,
  * not zero.  Builds the per-row search tables on the device (synchronises the device). */

@@ -28,7 +28,9 @@ EXPORTS = [
     "hcgrid_get_stats", "hcgrid_last_error", "hcgrid_debug_preorder",
     "hcgrid_debug_ang2pix_ring", "hcgrid_host_ang2pix_ring", "hcgrid_host_ring_info",
     "hcgrid_measure_peaks", "hcgrid_accumulate", "hcgrid_finalize", "hcgrid_accumulated_batches",
+    "hcgrid_set_kernel",
 ]
+KERNEL_GAUSS, KERNEL_TAPERED_SINC = 0, 1          # hcgrid_set_kernel types
 
 
 class HCGridError(RuntimeError):
@@ -67,6 +69,7 @@ def load_library():
     lib.hcgrid_create.argtypes = [ctypes.POINTER(vp), dbl, dbl, i64, ctypes.c_int, ctypes.c_int]
     lib.hcgrid_destroy.argtypes = [vp]
     lib.hcgrid_set_option.argtypes = [vp, ctypes.c_int, i64]
+    lib.hcgrid_set_kernel.argtypes = [vp, ctypes.c_int32, ctypes.c_double, ctypes.c_double]
     lib.hcgrid_set_target_car.argtypes = [vp, i32, i32, dbl, dbl, dbl, dbl]
     lib.hcgrid_set_target_cells.argtypes = [vp, i64, vp, vp, vp]
     lib.hcgrid_grid.argtypes = [vp, i64, vp, vp, vp, i32, vp, vp, vp, vp, vp]
@@ -186,6 +189,10 @@ class HCGrid:
     # -- configuration
     def set_option(self, option: int, value: int):
         self._check(self._lib.hcgrid_set_option(self._ctx, option, int(value)))
+
+    def set_kernel(self, kernel_type: int, a: float = 0.0, b: float = 0.0):
+        """hcgrid_set_kernel: KERNEL_GAUSS (default) or KERNEL_TAPERED_SINC with its a, b."""
+        self._check(self._lib.hcgrid_set_kernel(self._ctx, int(kernel_type), float(a), float(b)))
 
     def set_target_car(self, nx: int, ny: int, lon0_deg: float, lat0_deg: float, dlon_deg: float,
                        dlat_deg: float):

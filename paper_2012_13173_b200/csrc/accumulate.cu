@@ -31,7 +31,7 @@ finalize_kernel(const T* __restrict__ acc_cube, const T* __restrict__ acc_w, con
     if (i >= ncell * nchan) return;
     const int64_t cell = i / nchan;
     const T w = acc_w[cell];
-    cube[i] = w > (T)0 ? acc_cube[i] / w : nan;
+    cube[i] = w != (T)0 ? acc_cube[i] / w : nan;   // signed kernels: W may be negative
     if (i == cell * nchan) {
         wmap[cell] = w;
         if (counts) counts[cell] = acc_cnt[cell];

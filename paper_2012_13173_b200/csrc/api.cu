@@ -75,6 +75,8 @@ int hcgrid_create(hcgrid_ctx** out, double sigma_deg, double support_radius_deg,
     const double log2e = 1.4426950408889634074;
     kp.k1 = (float)(-log2e * kp.inv2s2);
     kp.k2 = (float)(-log2e * kp.inv2s2 / 12.0);
+    kp.ktype = HCGRID_KERNEL_GAUSS;
+    kp.inv_a2s2 = 0.0; kp.pi_bs = 0.0; kp.tg2 = 0.0f; kp.ts1 = 0.0f;
     *out = c;
     return HCGRID_OK;
 }
@@ -128,6 +130,26 @@ int hcgrid_set_option(hcgrid_ctx* c, int option, int64_t value) {
             break;
         default: return fail(c, HCGRID_ERR_INVALID_ARG, "unknown option %d", option);
     }
+    return HCGRID_OK;
+}
+
+int hcgrid_set_kernel(hcgrid_ctx* c, int32_t kernel_type, double a, double b) {
+    if (!c) return HCGRID_ERR_INVALID_ARG;
+    if (c->acc_nchan != 0)
+        return fail(c, HCGRID_ERR_INVALID_ARG, "the kernel cannot change while an accumulation is open");
+    KernelParams& kp = c->kp;
+    if (kernel_type == HCGRID_KERNEL_GAUSS) {
+        kp.ktype = HCGRID_KERNEL_GAUSS;
+        return HCGRID_OK;
+    }
+    if (kernel_type != HCGRID_KERNEL_TAPERED_SINC) return fail(c, HCGRID_ERR_INVALID_ARG, "unknown kernel type %d", (int)kernel_type);
+    if (!(a > 0.0) || !(b > 0.0) || !std::isfinite(a) || !std::isfinite(b))
+        return fail(c, HCGRID_ERR_INVALID_ARG, "tapered sinc needs a > 0 and b > 0");
+    kp.ktype = HCGRID_KERNEL_TAPERED_SINC;
+    kp.inv_a2s2 = 1.0 / (a * a * kp.sigma * kp.sigma);
+    kp.pi_bs = kPi / (b * kp.sigma);
+    kp.tg2 = (float)(2.0 / (a * a));
+    kp.ts1 = (float)(kPi * std::sqrt(2.0 * std::log(2.0)) / b);
     return HCGRID_OK;
 }
 

@@ -26,6 +26,24 @@ __device__ __forceinline__ T warp_sum(T x) {
     return x;
 }
 
+// Tapered sinc (PAPER.md:186 names the sinc; form of Winkel et al. 2016b, the work the paper
+// follows for its kernel set-up): sinc(d / (b sigma)) exp(-(d / (a sigma))^2), sinc(x) = sin(pi x)/(pi x).
+__device__ __forceinline__ double tapered_sinc64(double d2, const KernelParams& kp) {
+    const double y = sqrt(d2) * kp.pi_bs;
+    const double sinc = y == 0.0 ? 1.0 : sin(y) / y;
+    return sinc * exp(-d2 * kp.inv_a2s2);
+}
+
+// The same from the fp32 path's exponent: e2 = -t, t = d^2 log2e / (2 sigma^2) (what pair32
+// hands to ex2 for the Gaussian).  sinf, not the approximate intrinsic: the argument reaches
+// pi R / (b sigma) ~ 10 and the weight changes sign there.
+__device__ __forceinline__ float tapered_sinc32(float e2, const KernelParams& kp) {
+    const float t = fmaxf(-e2, 0.0f);
+    const float y = kp.ts1 * sqrtf(t);
+    const float sinc = y < 1e-4f ? 1.0f : sinf(y) / y;
+    return sinc * ex2_approx(-t * kp.tg2);
+}
+
 // fp64 pair: returns hit; w = q-less kernel weight.  The definition with no shortcut:
 // differences formed in degrees first, haversine, d = 2 asin(sqrt(hav)), w = exp(-d^2/(2 sigma^2)).
 __device__ __forceinline__ bool pair64(const Rec64& r, double clon_deg, double clat_deg, double ccos,
@@ -36,7 +54,7 @@ __device__ __forceinline__ bool pair64(const Rec64& r, double clon_deg, double c
     double hav = sa * sa + ccos * r.coslat * sb * sb;
     if (hav > 1.0) hav = 1.0;
     const double d = 2.0 * asin(sqrt(hav));
-    w = exp(-d * d * kp.inv2s2);
+    w = kp.ktype == 0 ? exp(-d * d * kp.inv2s2) : tapered_sinc64(d * d, kp);
     return d <= kp.radius;
 }
 
@@ -58,7 +76,7 @@ __device__ __forceinline__ bool pair64_small(const Rec64& r, double clon_deg, do
     const double dlon = remainder(r.lon_deg - clon_deg, 360.0) * kDeg2Rad;
     const double h = sin2_small(0.5 * dlat) + ccos * r.coslat * sin2_small(0.5 * dlon);
     const double d2 = 4.0 * h * fma(h, fma(h, fma(h, fma(h, 128.0 / 1575.0, 4.0 / 35.0), 8.0 / 45.0), 1.0 / 3.0), 1.0);
-    w = exp(-d2 * kp.inv2s2);
+    w = kp.ktype == 0 ? exp(-d2 * kp.inv2s2) : tapered_sinc64(d2, kp);
     return h <= kp.hav_max;
 }
 
@@ -114,8 +132,9 @@ conv_general(const ConvArgs a) {
                         const uint4 raw = __ldg((const uint4*)a.rec + sa + i);
                         Rec32 r;
                         r.xi = raw.x; r.yi = raw.y; r.idx = raw.z; r.q = __uint_as_float(raw.w);
-                        float wf;
-                        hit = pair32(r, tc, wf);
+                        float wf, e2;
+                        hit = pair32(r, tc, wf, &e2);
+                        if (a.kp.ktype != 0) wf = tapered_sinc32(e2, a.kp);
                         wq = (AccT)(wf * r.q);
                         idx = r.idx;
                     }
@@ -159,7 +178,7 @@ conv_general(const ConvArgs a) {
         const AccT nan = NanOf<AccT>::v();
         if (nchan == 1) {
             const AccT S = warp_sum(acc[0]);
-            if (lane == 0) cube[task] = a.raw ? S : (W > (AccT)0 ? S / W : nan);
+            if (lane == 0) cube[task] = a.raw ? S : (W != (AccT)0 ? S / W : nan);
         } else if (VEC4) {
 #pragma unroll
             for (int j = 0; j < 2; ++j) {
@@ -167,14 +186,14 @@ conv_general(const ConvArgs a) {
                 if (c < nchan) {
                     AccT* o = cube + (size_t)task * nchan + c;
 #pragma unroll
-                    for (int t = 0; t < 4; ++t) o[t] = a.raw ? acc[4 * j + t] : (W > (AccT)0 ? acc[4 * j + t] / W : nan);
+                    for (int t = 0; t < 4; ++t) o[t] = a.raw ? acc[4 * j + t] : (W != (AccT)0 ? acc[4 * j + t] / W : nan);
                 }
             }
         } else {
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
                 const int c = ch0 + lane + 32 * j;
-                if (c < nchan) cube[(size_t)task * nchan + c] = a.raw ? acc[j] : (W > (AccT)0 ? acc[j] / W : nan);
+                if (c < nchan) cube[(size_t)task * nchan + c] = a.raw ? acc[j] : (W != (AccT)0 ? acc[j] / W : nan);
             }
         }
         if (ch0 == 0 && lane == 0) {

@@ -101,6 +101,13 @@ struct KernelParams {      // per-context constants of the pair arithmetic
     double hav_max;                    // sin^2(R/2)
     float h4max;                       // 4 sin^2(R/2), rounded to fp32
     float k1, k2;                      // exponent = h4 * (k1 + k2 * h4): -log2e/(2 sigma^2) * (1, 1/12)
+    // kernel function (hcgrid_set_kernel): 0 Gaussian, 1 tapered sinc
+    //   sinc(d / (b sigma)) exp(-(d / (a sigma))^2),  sinc(x) = sin(pi x) / (pi x)
+    int ktype;
+    double inv_a2s2, pi_bs;            // 1 / (a sigma)^2,  pi / (b sigma)
+    float tg2, ts1;                    // fp32 path, from t = -exponent above = d^2 log2e / (2 sigma^2):
+                                       // taper = ex2(-t * tg2), tg2 = 2 / a^2; sinc argument = ts1 * sqrt(t),
+                                       // ts1 = pi sqrt(2 ln 2) / b
 };
 
 // ---------------------------------------------------------------- host-side helpers

@@ -77,7 +77,7 @@ __device__ __forceinline__ TaskConst make_task_const(const ConvArgs& a, const St
 
 // Step (v), one cell: fp32 pair arithmetic on exact fixed-point differences (see
 // pair_update in convolve.cu for the derivation).  Returns d <= R and the kernel weight.
-__device__ __forceinline__ bool pair32(const Rec32& r, const TaskConst& tc, float& w) {
+__device__ __forceinline__ bool pair32(const Rec32& r, const TaskConst& tc, float& w, float* e2_out = nullptr) {
     const float dx = (float)(int)(r.xi - tc.xc0) * tc.qx;
     const float dy = (float)(int)(r.yi - tc.yc) * tc.qy;
     const float u = dy * dy;
@@ -86,7 +86,9 @@ __device__ __forceinline__ bool pair32(const Rec32& r, const TaskConst& tc, floa
     const float v = dx * dx;
     const float B = v * fmaf(v, -1.0f / 12.0f, 1.0f);
     const float h4 = fmaf(C, B, u2);
-    w = ex2_approx(h4 * fmaf(h4, tc.k2, tc.k1));
+    const float e2 = h4 * fmaf(h4, tc.k2, tc.k1);     // -d^2 log2e / (2 sigma^2)
+    if (e2_out) *e2_out = e2;
+    w = ex2_approx(e2);
     return h4 <= tc.h4max;
 }
 
