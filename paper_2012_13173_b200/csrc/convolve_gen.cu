@@ -46,6 +46,7 @@ __device__ __forceinline__ float tapered_sinc32(float e2, const KernelParams& kp
 
 // fp64 pair: returns hit; w = q-less kernel weight.  The definition with no shortcut:
 // differences formed in degrees first, haversine, d = 2 asin(sqrt(hav)), w = exp(-d^2/(2 sigma^2)).
+template <int KFN>
 __device__ __forceinline__ bool pair64(const Rec64& r, double clon_deg, double clat_deg, double ccos,
                                        const KernelParams& kp, double& w) {
     const double dlat = (r.lat_deg - clat_deg) * kDeg2Rad;
@@ -54,7 +55,7 @@ __device__ __forceinline__ bool pair64(const Rec64& r, double clon_deg, double c
     double hav = sa * sa + ccos * r.coslat * sb * sb;
     if (hav > 1.0) hav = 1.0;
     const double d = 2.0 * asin(sqrt(hav));
-    w = kp.ktype == 0 ? exp(-d * d * kp.inv2s2) : tapered_sinc64(d * d, kp);
+    w = KFN == 0 ? exp(-d * d * kp.inv2s2) : tapered_sinc64(d * d, kp);
     return d <= kp.radius;
 }
 
@@ -70,17 +71,20 @@ __device__ __forceinline__ double sin2_small(double y) {
 // 4 h (1 + h/3 + 8 h^2/45 + 4 h^3/35 + ...), both exact to < 1e-16 relative there (h <= 6.3e-4), so the
 // result agrees with pair64 far inside the 1e-12 tier while costing a third of its fp64 instructions.
 // d <= R is tested as hav <= sin^2(R/2) (the same statement, asin and sqrt being monotone).
+template <int KFN>
 __device__ __forceinline__ bool pair64_small(const Rec64& r, double clon_deg, double clat_deg, double ccos,
                                              const KernelParams& kp, double& w) {
     const double dlat = (r.lat_deg - clat_deg) * kDeg2Rad;
     const double dlon = remainder(r.lon_deg - clon_deg, 360.0) * kDeg2Rad;
     const double h = sin2_small(0.5 * dlat) + ccos * r.coslat * sin2_small(0.5 * dlon);
     const double d2 = 4.0 * h * fma(h, fma(h, fma(h, fma(h, 128.0 / 1575.0, 4.0 / 35.0), 8.0 / 45.0), 1.0 / 3.0), 1.0);
-    w = kp.ktype == 0 ? exp(-d2 * kp.inv2s2) : tapered_sinc64(d2, kp);
+    w = KFN == 0 ? exp(-d2 * kp.inv2s2) : tapered_sinc64(d2, kp);
     return h <= kp.hav_max;
 }
 
-template <bool PAIR64, typename AccT, bool VEC4>
+// KFN: kernel function (hcgrid_set_kernel), 0 Gaussian, 1 tapered sinc -- a template parameter so
+// that the Gaussian instantiations carry none of the other's code.
+template <bool PAIR64, typename AccT, bool VEC4, int KFN>
 __global__ void __launch_bounds__(256)
 conv_general(const ConvArgs a) {
     const int lane = threadIdx.x & 31;
@@ -124,8 +128,8 @@ conv_general(const ConvArgs a) {
                     if (PAIR64) {
                         const Rec64 r = ((const Rec64*)a.rec)[sa + i];
                         double wd;
-                        hit = a.small64 ? pair64_small(r, clon_deg, clat_deg, ccos, a.kp, wd)
-                                        : pair64(r, clon_deg, clat_deg, ccos, a.kp, wd);
+                        hit = a.small64 ? pair64_small<KFN>(r, clon_deg, clat_deg, ccos, a.kp, wd)
+                                        : pair64<KFN>(r, clon_deg, clat_deg, ccos, a.kp, wd);
                         wq = (AccT)(wd * (double)r.q);
                         idx = r.idx;
                     } else {
@@ -134,7 +138,7 @@ conv_general(const ConvArgs a) {
                         r.xi = raw.x; r.yi = raw.y; r.idx = raw.z; r.q = __uint_as_float(raw.w);
                         float wf, e2;
                         hit = pair32(r, tc, wf, &e2);
-                        if (a.kp.ktype != 0) wf = tapered_sinc32(e2, a.kp);
+                        if (KFN != 0) wf = tapered_sinc32(e2, a.kp);
                         wq = (AccT)(wf * r.q);
                         idx = r.idx;
                     }
@@ -211,7 +215,11 @@ int launch_conv_general(hcgrid_ctx* c, const ConvArgs& a0, bool pair_f64, bool o
     const int threads = 256;
     const unsigned blocks = (unsigned)((a.ntasks + 7) / 8);
     if (blocks == 0) return HCGRID_OK;
-#define HCG_LAUNCH(P, T, V) conv_general<P, T, V><<<blocks, threads, 0, st>>>(a)
+#define HCG_LAUNCH(P, T, V)                                                        \
+    do {                                                                           \
+        if (a.kp.ktype == 0) conv_general<P, T, V, 0><<<blocks, threads, 0, st>>>(a); \
+        else conv_general<P, T, V, 1><<<blocks, threads, 0, st>>>(a);              \
+    } while (0)
     if (out_double) {
         if (vec4) HCG_LAUNCH(true, double, true); else HCG_LAUNCH(true, double, false);
     } else if (pair_f64) {
