@@ -304,10 +304,20 @@ int run_convolve(hcgrid_ctx* c, int64_t n, const float* values, int nchan, bool 
     c->stats.coarsen_y = 1;
     c->stats.split = 1;
     if (c->kp.ktype != 0) {
-        // kernel functions other than the paper's Gaussian live in the general kernels only
-        if (c->opt_kernel != 0 && c->opt_kernel != 2 && c->opt_kernel != 3)
-            return fail(c, HCGRID_ERR_UNSUPPORTED, "only the general kernels (HCGRID_OPT_KERNEL 0, 2, 3) evaluate "
-                        "kernel functions other than the Gaussian");
+        // kernel functions other than the paper's Gaussian: the tile kernel (one channel, plate-carree
+        // target, fp32 mode) and the general kernels
+        if (c->opt_kernel != 0 && c->opt_kernel != 2 && c->opt_kernel != 3 && c->opt_kernel != 5)
+            return fail(c, HCGRID_ERR_UNSUPPORTED, "only the tile and the general kernels (HCGRID_OPT_KERNEL 0, 2, 3, "
+                        "5) evaluate kernel functions other than the Gaussian");
+        if (f32 && nchan == 1 && c->tile_ok && (c->opt_kernel == 0 || c->opt_kernel == 5)) {
+            rc = launch_conv_tile(c, n, (float*)cube, (float*)wmap, counts, st);
+            c->stats.kernel = 6;
+            if (rc == HCGRID_OK) c->stats.gpu_launches += 1;
+            return rc;
+        }
+        if (c->opt_kernel == 5)
+            return fail(c, HCGRID_ERR_UNSUPPORTED, "the tile kernel needs fp32 mode, one channel and a plate-carree "
+                        "target whose reach is a plain longitude window");
         rc = launch_conv_general(c, a, !f32, c->precision == HCGRID_F64, st);
         c->stats.coarsen = 1;
         c->stats.kernel = f32 ? 3 : (c->precision == HCGRID_F64 ? 5 : 4);

@@ -27,7 +27,7 @@ namespace hcg {
 constexpr int kTileWarps = 4;        // warps (= tiles) per CTA when tiles are not split
 constexpr int kMaxTileWarps = 4;     // largest split: warps of one CTA on one tile
 
-template <int GX, int GY, int MODE, bool COUNTS, bool SPLIT>
+template <int GX, int GY, int MODE, bool COUNTS, bool SPLIT, int KFN = 0>
 __global__ void __launch_bounds__(kMaxTileWarps * 32)
 conv1_tile_f32(const TileArgs a) {
     constexpr int NC = GX * GY;
@@ -78,6 +78,7 @@ conv1_tile_f32(const TileArgs a) {
     tc.xc0 = (uint32_t)(unsigned long long)__double2ll_rn((a.u0 + (double)ix0 * a.du) * a.sx);
     tc.sxk = a.sxk; tc.syk = a.syk; tc.duk = a.duk; tc.dyk = a.dyk;
     tc.a12 = a.a12; tc.hmax = a.hmax;
+    tc.ts1 = a.ts1; tc.tg2 = a.tg2;
 
     float W[NC], S_[NC];
     int cnt[NC];
@@ -148,12 +149,12 @@ conv1_tile_f32(const TileArgs a) {
             const int ii = min(i, last);
             stream_seek(ii, tp, end, base);
             const uint4 rb = ldg_rec(base, ii);
-            tile_pairs<GX, GY, MODE, COUNTS>(ra, tc, W, S_, cnt);
+            tile_pairs<GX, GY, MODE, COUNTS, KFN>(ra, tc, W, S_, cnt);
             ra = rb;
         }
         if ((total & 31) && (nfull & (S - 1)) == part) {  // the ragged last step belongs to one warp
             tc.hm = i <= last ? tc.hmax : -1.0f;
-            tile_pairs<GX, GY, MODE, COUNTS>(ra, tc, W, S_, cnt);
+            tile_pairs<GX, GY, MODE, COUNTS, KFN>(ra, tc, W, S_, cnt);
         }
     }
 
@@ -179,7 +180,7 @@ conv1_tile_f32(const TileArgs a) {
         const int gx = c % GX, gy = c / GX;
         if (gx < ncols && gy < nrows) {
             const int64_t cell = (int64_t)(row0 + gy) * a.nx + ix0 + gx;
-            a.cube[cell] = a.raw ? ssum : (wsum > 0.0f ? ssum / wsum : __int_as_float(0x7fc00000));
+            a.cube[cell] = a.raw ? ssum : (wsum != 0.0f ? ssum / wsum : __int_as_float(0x7fc00000));
             a.wmap[cell] = wsum;
             if (COUNTS) a.counts[cell] = csum;
         }
@@ -208,14 +209,30 @@ static cudaError_t launch_shape(const TileArgs& a, int mode, bool counts, cudaSt
     return cudaGetLastError();
 }
 
+// Tapered sinc (KFN 1): series mode 2 only (valid wherever the tile kernel is), three shapes.
+template <int GX, int GY>
+static cudaError_t launch_shape_sinc(const TileArgs& a, bool counts, cudaStream_t st) {
+    const unsigned blocks = a.split > 1 ? (unsigned)a.ntiles : (unsigned)((a.ntiles + kTileWarps - 1) / kTileWarps);
+    const int threads = (a.split > 1 ? a.split : kTileWarps) * 32;
+    if (counts) {
+        if (a.split > 1) conv1_tile_f32<GX, GY, 2, true, true, 1><<<blocks, threads, 0, st>>>(a);
+        else conv1_tile_f32<GX, GY, 2, true, false, 1><<<blocks, threads, 0, st>>>(a);
+    } else {
+        if (a.split > 1) conv1_tile_f32<GX, GY, 2, false, true, 1><<<blocks, threads, 0, st>>>(a);
+        else conv1_tile_f32<GX, GY, 2, false, false, 1><<<blocks, threads, 0, st>>>(a);
+    }
+    return cudaGetLastError();
+}
+
 static const int kShapes[][2] = {{1, 1}, {2, 1}, {4, 1}, {8, 1}, {2, 2}, {4, 2}, {8, 2}, {4, 4}};
+static bool sinc_shape_built(int gx, int gy) { return (gx == 1 && gy == 1) || (gx == 2 && gy == 2) || (gx == 4 && gy == 2); }
 
 // Instruction-count model of one tile: warp instructions per cell.
 static double shape_cost(int gx, int gy, int mode, bool counts, double cw, double ch, double two_r,
-                         double ring_sp, double cand_per_cell) {
+                         double ring_sp, double cand_per_cell, bool sinc = false) {
     const double infl = (two_r + (gx - 1) * cw) / two_r * (two_r + 2.0 * ring_sp + (gy - 1) * ch) / (two_r + 2.0 * ring_sp);
     const double per_iter = 18.0 + (mode >= 1 ? 4.0 : 2.0) * gx + (mode >= 1 ? 5.0 : 3.0) * gy +
-                            (5.0 + (counts ? 1.0 : 0.0) + (mode == 2 ? 2.0 : 0.0)) * gx * gy;
+                            (5.0 + (counts ? 1.0 : 0.0) + (mode == 2 ? 2.0 : 0.0) + (sinc ? 45.0 : 0.0)) * gx * gy;
     const double iters = cand_per_cell * infl / 32.0 + 0.5;
     const double overhead = 150.0 + 14.0 * gy + 8.0 * gx * gy;
     // 16-cell tiles need ~100 registers per thread; measured on B200 they run 15-25 % slower than
@@ -258,7 +275,8 @@ int launch_conv_tile(hcgrid_ctx* c, int64_t n, float* cube, float* wmap, int32_t
     const Region& rg = c->region;
     const KernelParams& kp = c->kp;
     const int nx = c->strip_cells, ny = c->nstrip;
-    const int mode = tile_series_mode(c);
+    const bool sinc = kp.ktype == HCGRID_KERNEL_TAPERED_SINC;
+    const int mode = sinc ? 2 : tile_series_mode(c);
 
     // tile shape: forced by the options or chosen by the instruction-count model
     int gx = c->opt_coarsen, gy = c->opt_coarsen_y;
@@ -274,8 +292,9 @@ int launch_conv_tile(hcgrid_ctx* c, int64_t n, float* cube, float* wmap, int32_t
             if ((gx != 0 && s[0] != gx) || (gy != 0 && s[1] != gy)) continue;
             if (s[0] > nx && s[0] > 1) continue;
             if (s[1] > ny && s[1] > 1) continue;
+            if (sinc && !sinc_shape_built(s[0], s[1])) continue;
             const double cost = shape_cost(s[0], s[1], mode, counts != nullptr, c->cell_width_sky,
-                                           std::fabs(c->car_dlat), two_r, ring_sp, cand);
+                                           std::fabs(c->car_dlat), two_r, ring_sp, cand, sinc);
             if (cost < best) { best = cost; bx = s[0]; by = s[1]; }
         }
         if (best == 1e300)
@@ -307,10 +326,17 @@ int launch_conv_tile(hcgrid_ctx* c, int64_t n, float* cube, float* wmap, int32_t
 
     cudaError_t e = cudaSuccess;
     bool built = false;
-#define HCG_SHAPE(X, Y) if (gx == X && gy == Y) { built = true; e = launch_shape<X, Y>(a, mode, counts != nullptr, st); }
-    HCG_SHAPE(1, 1); HCG_SHAPE(2, 1); HCG_SHAPE(4, 1); HCG_SHAPE(8, 1);
-    HCG_SHAPE(2, 2); HCG_SHAPE(4, 2); HCG_SHAPE(8, 2); HCG_SHAPE(4, 4);
+    if (sinc) {
+        a.ts1 = kp.ts1; a.tg2 = kp.tg2;
+#define HCG_SHAPE(X, Y) if (gx == X && gy == Y) { built = true; e = launch_shape_sinc<X, Y>(a, counts != nullptr, st); }
+        HCG_SHAPE(1, 1); HCG_SHAPE(2, 2); HCG_SHAPE(4, 2);
 #undef HCG_SHAPE
+    } else {
+#define HCG_SHAPE(X, Y) if (gx == X && gy == Y) { built = true; e = launch_shape<X, Y>(a, mode, counts != nullptr, st); }
+        HCG_SHAPE(1, 1); HCG_SHAPE(2, 1); HCG_SHAPE(4, 1); HCG_SHAPE(8, 1);
+        HCG_SHAPE(2, 2); HCG_SHAPE(4, 2); HCG_SHAPE(8, 2); HCG_SHAPE(4, 4);
+#undef HCG_SHAPE
+    }
     if (!built)
         return fail(c, HCGRID_ERR_INVALID_ARG, "tile shape %d x %d not built", gx, gy);
     if (e != cudaSuccess) return cuda_fail(c, e, "conv1_tile_f32");

@@ -25,6 +25,7 @@ struct TileArgs {
     float isk;                  // 1 / sqrt(kappa)
     float a12;                  // 1 / (12 kappa): series coefficient in scaled units
     float hmax;                 // kappa * 4 sin^2(R/2)  (series modes)  or  kappa * R^2 (flat mode)
+    float ts1, tg2;             // tapered sinc (KFN 1): sinc argument = ts1 sqrt(e), taper = ex2(-e tg2)
 };
 
 template <int GY>
@@ -35,12 +36,34 @@ struct TileConst {
     float cc[GY];
     float a12, hmax;
     float hm;                   // hmax, or -1 for a lane that is past the end of the stream
+    float ts1, tg2;             // KFN 1 only
 };
+
+// Tapered sinc from e = kappa d^2 (the Gaussian's base-2 exponent): sinc(ts1 sqrt(e)) ex2(-e tg2).
+// sin by hand: y = k pi + r, |r| <= pi/2 (pi split in two so that k pi is exact for the k <= ~30 the
+// support radius allows), odd Taylor polynomial to r^11 (next term r^13/13! <= 5.7e-8), sign from k's parity.
+__device__ __forceinline__ float tile_tapered_sinc(float e, float ts1, float tg2) {
+    const float y = ts1 * sqrtf(e);
+    const float kb = fmaf(y, 0.318309886f, 12582912.0f);          // 1.5 * 2^23: the integer lands in the low bits
+    const float k = kb - 12582912.0f;
+    float r = fmaf(k, -3.140625f, y);
+    r = fmaf(k, -9.67653589793e-4f, r);
+    const float r2 = r * r;
+    float p = fmaf(r2, -2.50521084e-8f, 2.75573192e-6f);
+    p = fmaf(r2, p, -1.98412698e-4f);
+    p = fmaf(r2, p, 8.33333333e-3f);
+    p = fmaf(r2, p, -1.66666667e-1f);
+    p = fmaf(r2 * r, p, r);
+    const float s = __uint_as_float(__float_as_uint(p) ^ (__float_as_uint(kb) << 31));
+    const float sinc = y < 1e-4f ? 1.0f : __fdividef(s, y);
+    return sinc * ex2_approx(-e * tg2);
+}
 
 // MODE 0 "flat": d^2 = dy^2 + cos cos dx^2 (valid while R^2/12 and dl_max^2/12 < 1e-7);
 // MODE 1 "series": 4 hav(d) = u(1-u/12) + C v(1-v/12) for the test, weight from the same;
 // MODE 2 "full": as 1, plus d^2 = h(1 + h/12) for the weight.
-template <int GX, int GY, int MODE, bool COUNTS>
+// KFN 0: Gaussian, w = ex2(-e); KFN 1: tapered sinc of the same e (hcgrid_set_kernel).
+template <int GX, int GY, int MODE, bool COUNTS, int KFN = 0>
 __device__ __forceinline__ void tile_pairs(const uint4 raw, const TileConst<GY>& tc, float (&W)[GX * GY],
                                            float (&S)[GX * GY], int (&cnt)[GX * GY]) {
     const float q = __uint_as_float(raw.w);
@@ -68,7 +91,7 @@ __device__ __forceinline__ void tile_pairs(const uint4 raw, const TileConst<GY>&
         for (int i = 0; i < GX; ++i) {
             const float h = fmaf(C[j], V[i], U[j]);
             const float e = MODE == 2 ? h * fmaf(h, tc.a12, 1.0f) : h;
-            const float w = ex2_approx(-e);
+            const float w = KFN == 0 ? ex2_approx(-e) : tile_tapered_sinc(fmaxf(e, 0.0f), tc.ts1, tc.tg2);
             // predicated accumulate, spelled out so the count stays one predicated add
             if (COUNTS)
                 asm("{\n\t.reg .pred p;\n\t"

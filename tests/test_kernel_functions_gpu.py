@@ -76,7 +76,8 @@ def test_tapered_sinc_config_miniatures(oracle, cfg, precision):
     w = workloads.make(cfg, MINI[cfg])
     ref = _oracle(oracle, w, (oracle.TAPERED_SINC, A, B))
     cube, wmap, cnt, st = _gpu(w, precision, (1, A, B))
-    assert st["kernel"] in (3, 5)                       # the general kernels
+    # fp32, one channel, plate-carree: the tile kernel; otherwise the general kernels
+    assert st["kernel"] == (6 if precision == "f32" and w.nchan == 1 else (3 if precision == "f32" else 5))
     r = _cmp(cube, wmap, cnt, ref, w, precision)
     assert r["cells_compared"] > 0.5 * w.target.ncell
 
@@ -102,6 +103,24 @@ def test_tapered_sinc_negative_weight_cells_and_arbitrary_cells(oracle, precisio
     assert np.all(np.isfinite(cube[neg]))
 
 
+@pytest.mark.parametrize("cfg", [1, 3, 5])
+@pytest.mark.parametrize("variant", ["general", "tile1x1", "tile2x2", "tile4x2", "tile4x2split2"])
+def test_tapered_sinc_kernel_variants(oracle, cfg, variant):
+    from paper_2012_13173_b200 import binding
+    w = workloads.make(cfg, MINI[cfg])
+    ref = _oracle(oracle, w, (oracle.TAPERED_SINC, A, B))
+    if variant == "general":
+        opts, want = {binding.OPT_KERNEL: binding.KERNEL_GENERAL}, 3
+    else:
+        gx, gy = int(variant[4]), int(variant[6])
+        opts, want = {binding.OPT_KERNEL: binding.KERNEL_TILE, binding.OPT_COARSEN: gx, binding.OPT_COARSEN_Y: gy}, 6
+        if variant.endswith("split2"):
+            opts[binding.OPT_SPLIT] = 2
+    cube, wmap, cnt, st = _gpu(w, "f32", (1, A, B), options=opts)
+    assert st["kernel"] == want
+    _cmp(cube, wmap, cnt, ref, w, "f32")
+
+
 def test_tapered_sinc_with_huge_b_is_the_gaussian_path(oracle):
     """b -> infinity leaves exp(-(d / (a sigma))^2): the general kernel's tapered-sinc branch must then
     agree with the Gaussian oracle of width a sigma / sqrt 2 at the ordinary 1e-5 bar."""
@@ -123,12 +142,12 @@ def test_set_kernel_switches_back_and_validates(oracle):
             g.set_kernel(*bad)
     lon, lat, val = _dev(w.lon), _dev(w.lat), _dev(w.values)
     g.set_kernel(binding.KERNEL_TAPERED_SINC, A, B)
-    g.set_option(binding.OPT_KERNEL, binding.KERNEL_TILE)
-    with pytest.raises(binding.HCGridError):            # tile kernel evaluates the Gaussian only
+    g.set_option(binding.OPT_KERNEL, binding.KERNEL_STAGED)
+    with pytest.raises(binding.HCGridError):            # the staged kernel evaluates the Gaussian only
         g.grid(lon, lat, val)
     g.set_option(binding.OPT_KERNEL, binding.KERNEL_AUTO)
     c1, w1, n1 = g.grid(lon, lat, val)
-    assert g.stats()["kernel"] == 3
+    assert g.stats()["kernel"] == 6
     g.set_kernel(binding.KERNEL_GAUSS)
     c0, w0, n0 = g.grid(lon, lat, val)
     torch.cuda.synchronize()
