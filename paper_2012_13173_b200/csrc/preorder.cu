@@ -116,18 +116,29 @@ tables_pack_kernel(const uint32_t* __restrict__ skeys, const uint32_t* __restric
 // The keys are bin numbers of a table that is built anyway, so the sort of PAPER.md:120 is a
 // counting sort: pixelise_kernel<.., true> counts every bin and keeps each sample's arrival
 // rank, an exclusive scan of the counts IS bin_start (a4), scatter_index_kernel puts sample i
-// at bin_start[key] + rank, and bin_order_kernel puts every bin's indices in ascending order
-// -- arrival order is whatever the atomics made it; ascending index is what the stable sort
-// gives, so S' is identical to the radix path's, bit for bit.  pack32_kernel gathers (a5).
+// at bin_start[key] + rank, and order_pack_kernel moves every index to its place in ascending
+// order inside its bin -- arrival order is whatever the atomics made it; ascending index is what
+// the stable sort gives, so S' is identical to the radix path's, bit for bit -- gathering the
+// record on the way (a5).
 
+constexpr int kLongBin = 1024;           // bins longer than this are ordered by the block-sort kernel
+constexpr uint32_t kStartFlag = 0x80000000u, kIdxMask = 0x7fffffffu;   // n <= 2e9 < 2^31 (hcgrid_grid)
+
+// sidx_raw[bin_start[key] + rank] = i, with the top bit set on rank 0: the sample that arrived
+// first sits at its bin's first position and so marks where the bin begins.  The one sample
+// with rank == kLongBin (there is exactly one iff the bin is longer) queues its bin for the
+// block-sort kernel.
 __global__ void __launch_bounds__(256)
 scatter_index_kernel(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ rank, int64_t n,
-                     int32_t nbins, const int32_t* __restrict__ bin_start, uint32_t* __restrict__ sidx) {
+                     int32_t nbins, const int32_t* __restrict__ bin_start, uint32_t* __restrict__ sidx_raw,
+                     int32_t* __restrict__ long_count, int32_t* __restrict__ long_list) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const uint32_t key = keys[i];
     if (key >= (uint32_t)nbins) return;
-    sidx[(int64_t)__ldg(bin_start + key) + rank[i]] = (uint32_t)i;
+    const uint32_t r = rank[i];
+    sidx_raw[(int64_t)__ldg(bin_start + key) + r] = (uint32_t)i | (r == 0 ? kStartFlag : 0u);
+    if (r == (uint32_t)kLongBin) long_list[atomicAdd(long_count, 1)] = (int32_t)key;
 }
 
 // Ascending sort of a[0, L) by the whole block, in place in global memory: the bitonic
@@ -159,77 +170,61 @@ __device__ void block_sort_u32(uint32_t* a, int L, int tid, int nthr) {
     }
 }
 
-constexpr int kInsertReach = 48;     // positions an index may travel in the thread-serial pass
-
-// Thread b owns bin b: orders sidx[bin_start[b], bin_start[b+1]) ascending.  Bins the thread
-// cannot finish (see below) are queued in shared memory and sorted by the whole block.
+// a3 (order inside the bins) + a5 in one pass, one thread per position p of the arrival-ordered
+// index array: the thread walks left to its bin's start flag and right to the next one, counting
+// on the way how many of the bin's indices are smaller than its own -- that count is its place in
+// ascending order, which is the stable sort's order -- and writes its index (and, kPack, the
+// gathered record) there.  The walks are neighbouring loads the warp has in L1 anyway; the kernel
+// stays bound by the random record gather.  Bins longer than kLongBin are left to order_long_kernel.
+template <bool kPack>
 __global__ void __launch_bounds__(256)
-bin_order_kernel(int32_t nbins, const int32_t* __restrict__ bin_start, uint32_t* sidx) {
-    __shared__ int s_cnt;
-    __shared__ int s_lo[256], s_len[256];
-    const int tid = threadIdx.x;
-    const int64_t b = (int64_t)blockIdx.x * blockDim.x + tid;
-    if (tid == 0) s_cnt = 0;
-    __syncthreads();
-    if (b < nbins) {
-        const int s = bin_start[b], e = bin_start[b + 1];
-        const int cnt = e - s;
-        if (cnt > 8) {
-            // Arrival order follows launch order up to the samples in flight together, so a
-            // long bin is ascending but for short-range disorder: one insertion pass with the
-            // running maximum in a register and a bounded reach.  Whoever needs to travel
-            // further than kInsertReach sends the bin to the block sort below.
-            bool far = false;
-            uint32_t top = sidx[s];
-            for (int a = s + 1; a < e; ++a) {
-                const uint32_t v = sidx[a];
-                if (v >= top) { top = v; continue; }
-                int p = a;
-                const int stop = max(s, a - kInsertReach);
-                while (p > stop) {
-                    const uint32_t u = sidx[p - 1];
-                    if (u <= v) break;
-                    sidx[p] = u;
-                    --p;
-                }
-                sidx[p] = v;
-                far |= p == stop && p > s && sidx[p - 1] > v;
-            }
-            if (far) {
-                const int slot = atomicAdd(&s_cnt, 1);
-                s_lo[slot] = s; s_len[slot] = cnt;
-            }
-        } else if (cnt >= 2 && cnt <= 8) {
-            // up to 8: registers and a fixed 19-comparator network (Batcher's merge exchange),
-            // one memory round trip whatever the count; the padding sorts to the top
-            uint32_t v[8];
-#pragma unroll
-            for (int k = 0; k < 8; ++k) v[k] = k < cnt ? sidx[s + k] : 0xffffffffu;
-#define HCG_CX(i, j) { const uint32_t lo_ = min(v[i], v[j]), hi_ = max(v[i], v[j]); v[i] = lo_; v[j] = hi_; }
-            HCG_CX(0, 1) HCG_CX(2, 3) HCG_CX(4, 5) HCG_CX(6, 7)
-            HCG_CX(0, 2) HCG_CX(1, 3) HCG_CX(4, 6) HCG_CX(5, 7)
-            HCG_CX(1, 2) HCG_CX(5, 6)
-            HCG_CX(0, 4) HCG_CX(1, 5) HCG_CX(2, 6) HCG_CX(3, 7)
-            HCG_CX(2, 4) HCG_CX(3, 5)
-            HCG_CX(1, 2) HCG_CX(3, 4) HCG_CX(5, 6)
-#undef HCG_CX
-#pragma unroll
-            for (int k = 0; k < 8; ++k)
-                if (k < cnt) sidx[s + k] = v[k];
-        }
+order_pack_kernel(const uint32_t* __restrict__ sidx_raw, int64_t n, const int32_t* __restrict__ nkept_ptr,
+                  uint32_t* __restrict__ sidx, const Rec32* __restrict__ rec_in, Rec32* __restrict__ rec_out) {
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t nkept = nkept_ptr[0];
+    if (p >= n || p >= nkept) return;
+    const uint32_t raw = sidx_raw[p];
+    const uint32_t v = raw & kIdxMask;
+    int below = 0;
+    int64_t s = p;
+    uint32_t x = raw;
+    while (!(x & kStartFlag)) {
+        if (p - s >= kLongBin) return;                       // a long bin
+        --s;
+        x = sidx_raw[s];
+        below += (x & kIdxMask) < v;
     }
-    __syncthreads();
-    const int nq = s_cnt;
-    for (int g = 0; g < nq; ++g) block_sort_u32(sidx + s_lo[g], s_len[g], tid, 256);
+    int64_t e = p + 1;
+    while (e < nkept) {
+        x = sidx_raw[e];
+        if (x & kStartFlag) break;
+        if (e - s >= kLongBin) return;                       // a long bin (every member sees the same length)
+        below += (x & kIdxMask) < v;
+        ++e;
+    }
+    const int64_t d = s + below;
+    sidx[d] = v;
+    if (kPack) *(uint4*)(rec_out + d) = __ldg((const uint4*)(rec_in + v));
 }
 
-// a5 after the counting sort: rec_out[p] = rec_in[sidx[p]] for p < nkept = bin_start[nbins].
+// The queued long bins, one block at a time: copy the indices, sort them (block_sort_u32), gather.
+template <bool kPack>
 __global__ void __launch_bounds__(256)
-pack32_kernel(const uint32_t* __restrict__ sidx, int64_t n, const int32_t* __restrict__ nkept,
-              const Rec32* __restrict__ rec_in, Rec32* __restrict__ rec_out) {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n || i >= (int64_t)nkept[0]) return;
-    *(uint4*)(rec_out + i) = __ldg((const uint4*)(rec_in + sidx[i]));
+order_long_kernel(const uint32_t* __restrict__ sidx_raw, const int32_t* __restrict__ bin_start,
+                  const int32_t* __restrict__ long_count, const int32_t* __restrict__ long_list, uint32_t* sidx,
+                  const Rec32* __restrict__ rec_in, Rec32* __restrict__ rec_out) {
+    const int nlong = long_count[0];
+    for (int g = blockIdx.x; g < nlong; g += gridDim.x) {
+        const int key = long_list[g];
+        const int s = bin_start[key], len = bin_start[key + 1] - s;
+        for (int k = threadIdx.x; k < len; k += 256) sidx[s + k] = sidx_raw[s + k] & kIdxMask;
+        __syncthreads();
+        block_sort_u32(sidx + s, len, threadIdx.x, 256);    // ends with a barrier
+        if (kPack)
+            for (int k = threadIdx.x; k < len; k += 256)
+                *(uint4*)(rec_out + s + k) = __ldg((const uint4*)(rec_in + sidx[s + k]));
+        __syncthreads();
+    }
 }
 
 __global__ void __launch_bounds__(256)
@@ -269,11 +264,12 @@ int run_preorder(hcgrid_ctx* c, int64_t n, const double* lon, const double* lat,
     int end_bit = 1;
     while (end_bit < 32 && ((uint64_t)1 << end_bit) <= (uint64_t)rg.nbins) ++end_bit;
     size_t tmp_bytes = 0;
+    HCG_CUDA(c, c->d_keys_out.ensure(nn * 4));
     if (counting) {
+        HCG_CUDA(c, c->d_long.ensure((nn / kLongBin + 2) * 4));
         HCG_CUDA(c, cub::DeviceScan::ExclusiveSum(nullptr, tmp_bytes, c->d_bins.as<int32_t>(), c->d_bins.as<int32_t>(),
                                                   (int64_t)rg.nbins + 1, st));
     } else {
-        HCG_CUDA(c, c->d_keys_out.ensure(nn * 4));
         HCG_CUDA(c, cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, c->d_keys.as<uint32_t>(),
                                                     c->d_keys_out.as<uint32_t>(), c->d_idx.as<uint32_t>(),
                                                     c->d_idx_out.as<uint32_t>(), (int64_t)nn, 0, end_bit, st));
@@ -289,8 +285,9 @@ int run_preorder(hcgrid_ctx* c, int64_t n, const double* lon, const double* lat,
         int32_t* bins = c->d_bins.as<int32_t>();
         uint32_t* keys = c->d_keys.as<uint32_t>();
         uint32_t* rank = c->d_idx.as<uint32_t>();
-        uint32_t* sidx = c->d_idx_out.as<uint32_t>();
-        HCG_CUDA(c, cudaMemsetAsync(bins, 0, ((size_t)rg.nbins + 1) * 4, st));
+        uint32_t* sidx_raw = c->d_keys_out.as<uint32_t>();   // arrival order, start-of-bin flags
+        uint32_t* sidx = c->d_idx_out.as<uint32_t>();        // ascending inside every bin: the sorted "value" column
+        HCG_CUDA(c, cudaMemsetAsync(bins, 0, ((size_t)rg.nbins + 2) * 4, st));
         if (f32)
             pixelise_kernel<true, true><<<nb, threads, 0, st>>>(lon, lat, values, weights, nchan, n, rg, keys, rank,
                                                                 c->d_misc.as<Rec32>(), bins);
@@ -300,19 +297,25 @@ int run_preorder(hcgrid_ctx* c, int64_t n, const double* lon, const double* lat,
         HCG_CUDA(c, cudaGetLastError());
         if (c->opt_profile) cudaEventRecord(c->ev[1], st);
         HCG_CUDA(c, cub::DeviceScan::ExclusiveSum(c->d_sort_tmp.p, tmp_bytes, bins, bins, (int64_t)rg.nbins + 1, st));
-        scatter_index_kernel<<<nb, threads, 0, st>>>(keys, rank, n, (int32_t)rg.nbins, bins, sidx);
+        int32_t* long_count = bins + rg.nbins + 1;           // spare entry of the table, zeroed with it
+        int32_t* long_list = c->d_long.as<int32_t>();
+        scatter_index_kernel<<<nb, threads, 0, st>>>(keys, rank, n, (int32_t)rg.nbins, bins, sidx_raw, long_count,
+                                                     long_list);
         HCG_CUDA(c, cudaGetLastError());
-        if (c->opt_profile) cudaEventRecord(c->ev[2], st);
-        const unsigned nbb = (unsigned)(((size_t)rg.nbins + threads - 1) / threads);
-        bin_order_kernel<<<nbb, threads, 0, st>>>((int32_t)rg.nbins, bins, sidx);
-        HCG_CUDA(c, cudaGetLastError());
-        launches = 5;                        // pixelise, scan (2 kernels), scatter, order
-        if (c->opt_profile) cudaEventRecord(c->ev[3], st);
+        if (c->opt_profile) { cudaEventRecord(c->ev[2], st); cudaEventRecord(c->ev[3], st); }
+        const unsigned nlb = (unsigned)(4 * c->num_sms);
         if (f32) {
-            pack32_kernel<<<nb, threads, 0, st>>>(sidx, n, bins + rg.nbins, c->d_misc.as<Rec32>(), c->d_rec.as<Rec32>());
-            ++launches;
-            HCG_CUDA(c, cudaGetLastError());
+            order_pack_kernel<true><<<nb, threads, 0, st>>>(sidx_raw, n, bins + rg.nbins, sidx, c->d_misc.as<Rec32>(),
+                                                            c->d_rec.as<Rec32>());
+            order_long_kernel<true><<<nlb, threads, 0, st>>>(sidx_raw, bins, long_count, long_list, sidx,
+                                                             c->d_misc.as<Rec32>(), c->d_rec.as<Rec32>());
+        } else {
+            order_pack_kernel<false><<<nb, threads, 0, st>>>(sidx_raw, n, bins + rg.nbins, sidx, nullptr, nullptr);
+            order_long_kernel<false><<<nlb, threads, 0, st>>>(sidx_raw, bins, long_count, long_list, sidx, nullptr,
+                                                              nullptr);
         }
+        HCG_CUDA(c, cudaGetLastError());
+        launches = 6;                        // pixelise, scan (2 kernels), scatter, order + pack, long bins
     } else {
         if (n > 0) {
             if (f32)
