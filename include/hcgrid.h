@@ -70,7 +70,7 @@ enum {
     HCGRID_OPT_COARSEN_Y = 6,    /* target rows per warp task (tile kernel); 0 = auto */
     HCGRID_OPT_SPLIT = 7,        /* warps sharing one tile's candidate stream (tile kernel): 1, 2, 4; 0 = auto */
     HCGRID_OPT_PREORDER = 8      /* how S' is ordered: 1 = radix sort of (key, n); 2 = counting sort into the
-                                    bin table (same S', bit for bit); 0 = auto (counting up to 16 samples per bin) */
+                                    bin table (same S', bit for bit); 0 = auto (counting up to 10 samples per bin) */
 };
 
 typedef struct {

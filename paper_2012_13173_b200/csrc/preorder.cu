@@ -252,7 +252,7 @@ int run_preorder(hcgrid_ctx* c, int64_t n, const double* lon, const double* lat,
     // the same S' either way
     const int64_t nbins64 = (int64_t)rg.nbins;
     const bool counting = n > 0 && (c->opt_preorder == 2 ||
-                                    (c->opt_preorder == 0 && n <= 16 * nbins64 &&
+                                    (c->opt_preorder == 0 && n <= 10 * nbins64 &&
                                      (nbins64 <= 16 * n || nbins64 <= ((int64_t)1 << 22))));
     const size_t nn = (size_t)(n > 0 ? n : 1);
     HCG_CUDA(c, c->d_keys.ensure(nn * 4));

@@ -159,4 +159,4 @@ def test_preorder_auto_choice():
     lat = np.tile(w.lat, 40)
     val = np.tile(w.values, (40, 1))
     st2 = _run_preorder_mode(w, binding.PREORDER_AUTO, lon=lon, lat=lat, values=val)[4]
-    assert st2["preorder"] == (2 if lon.size <= 16 * st2["n_bins"] else 1)
+    assert st2["preorder"] == (2 if lon.size <= 10 * st2["n_bins"] else 1)
