@@ -69,6 +69,9 @@ enum {
     HCGRID_OPT_WARPS_PER_SM = 5, /* resident convolution warps per SM (staged kernel); 0 = auto */
     HCGRID_OPT_COARSEN_Y = 6,    /* target rows per warp task (tile kernel); 0 = auto */
     HCGRID_OPT_SPLIT = 7,        /* warps sharing one tile's candidate stream (tile kernel): 1, 2, 4; 0 = auto */
+    HCGRID_OPT_HOST_CHUNKS = 9,  /* hcgrid_grid_host: pieces the samples are copied and gridded in (copy of piece
+                                    k+1 overlaps the gridding of piece k); 1 = one copy, one hcgrid_grid; 0 = auto
+                                    (4 from 64 MB of input) */
     HCGRID_OPT_PREORDER = 8      /* how S' is ordered: 1 = radix sort of (key, n); 2 = counting sort into the
                                     bin table (same S', bit for bit); 0 = auto (counting up to 10 samples per bin) */
 };
@@ -134,7 +137,13 @@ int hcgrid_grid(hcgrid_ctx* ctx, int64_t n, const double* lon_deg, const double*
                 void* datacube, void* weightmap, int32_t* counts, void* stream);
 
 /* Same call with HOST buffers (pinned or pageable): copies the inputs to context-owned
- * device buffers, grids, copies the outputs back and synchronises before returning. */
+ * device buffers, grids, copies the outputs back and synchronises before returning.
+ * From 64 MB of input on (HCGRID_OPT_HOST_CHUNKS) the samples go over in 4 pieces on a copy
+ * stream while a second stream grids the pieces that have arrived (hcgrid_accumulate on each,
+ * one hcgrid_finalize): the same sums added in a different order, so the result agrees with
+ * hcgrid_grid's to rounding, not bit for bit; it is deterministic for a given piece count.
+ * Pinned buffers are needed for the copies to overlap anything.  Falls back to one piece while
+ * the caller has an accumulation open. */
 int hcgrid_grid_host(hcgrid_ctx* ctx, int64_t n, const double* lon_deg, const double* lat_deg,
                      const float* values, int32_t nchan, const float* weights,
                      void* datacube, void* weightmap, int32_t* counts);

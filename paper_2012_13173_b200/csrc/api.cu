@@ -91,6 +91,9 @@ int hcgrid_destroy(hcgrid_ctx* c) {
                       &c->d_tmp_cnt};
     for (DevBuf* b : bufs) b->release();
     for (auto& ev : c->ev) if (ev) cudaEventDestroy(ev);
+    for (auto& ev : c->ev_chunk) if (ev) cudaEventDestroy(ev);
+    if (c->st_copy) cudaStreamDestroy(c->st_copy);
+    if (c->st_comp) cudaStreamDestroy(c->st_comp);
     delete c;
     return HCGRID_OK;
 }
@@ -123,6 +126,10 @@ int hcgrid_set_option(hcgrid_ctx* c, int option, int64_t value) {
             if (value != 0 && value != 1 && value != 2 && value != 4)
                 return fail(c, HCGRID_ERR_INVALID_ARG, "split must be 0 (auto), 1, 2 or 4");
             c->opt_split = (int)value;
+            break;
+        case HCGRID_OPT_HOST_CHUNKS:
+            if (value < 0 || value > 16) return fail(c, HCGRID_ERR_INVALID_ARG, "host chunks must be 0 (auto) or 1..16");
+            c->opt_host_chunks = (int)value;
             break;
         case HCGRID_OPT_PREORDER:
             if (value < 0 || value > 2) return fail(c, HCGRID_ERR_INVALID_ARG, "preorder must be 0 (auto), 1 or 2");
@@ -220,6 +227,47 @@ int hcgrid_grid_host(hcgrid_ctx* c, int64_t n, const double* lon, const double* 
     HCG_CUDA(c, c->d_out_cube.ensure(nc * (size_t)nchan * osz));
     HCG_CUDA(c, c->d_out_w.ensure(nc * osz));
     if (counts) HCG_CUDA(c, c->d_out_cnt.ensure(nc * 4));
+    // Large inputs: the copy is most of the call (PCIe), so the samples go over in chunks on one
+    // stream while a second stream grids the chunks that have arrived -- Eq. 1's two sums are
+    // additive over samples (hcgrid_accumulate), the division happens once at the end.
+    int chunks = c->opt_host_chunks;
+    if (chunks == 0) chunks = nn * (20 + 4 * (size_t)nchan) >= ((size_t)64 << 20) ? 4 : 1;
+    if (c->acc_nchan != 0 || n < 4096) chunks = 1;          // an open accumulation is the caller's
+    if (chunks > 1) {
+        if (!c->st_copy) HCG_CUDA(c, cudaStreamCreateWithFlags(&c->st_copy, cudaStreamNonBlocking));
+        if (!c->st_comp) HCG_CUDA(c, cudaStreamCreateWithFlags(&c->st_comp, cudaStreamNonBlocking));
+        for (int k = 0; k < chunks; ++k)
+            if (!c->ev_chunk[k]) HCG_CUDA(c, cudaEventCreateWithFlags(&c->ev_chunk[k], cudaEventDisableTiming));
+        HCG_CUDA(c, cudaDeviceSynchronize());               // scratch may still be in use on the caller's streams
+        const int64_t per = ((n + chunks - 1) / chunks + 63) & ~(int64_t)63;   // keeps value rows 16-byte aligned
+        for (int k = 0; k < chunks; ++k) {
+            const int64_t lo = std::min<int64_t>(n, (int64_t)k * per), hi = std::min<int64_t>(n, lo + per);
+            const size_t m = (size_t)(hi - lo);
+            if (m > 0) {
+                HCG_CUDA(c, cudaMemcpyAsync(c->d_in_lon.as<double>() + lo, lon + lo, m * 8, cudaMemcpyHostToDevice, c->st_copy));
+                HCG_CUDA(c, cudaMemcpyAsync(c->d_in_lat.as<double>() + lo, lat + lo, m * 8, cudaMemcpyHostToDevice, c->st_copy));
+                HCG_CUDA(c, cudaMemcpyAsync(c->d_in_val.as<float>() + (size_t)lo * nchan, values + (size_t)lo * nchan,
+                                            m * (size_t)nchan * 4, cudaMemcpyHostToDevice, c->st_copy));
+                if (weights)
+                    HCG_CUDA(c, cudaMemcpyAsync(c->d_in_wgt.as<float>() + lo, weights + lo, m * 4, cudaMemcpyHostToDevice, c->st_copy));
+            }
+            HCG_CUDA(c, cudaEventRecord(c->ev_chunk[k], c->st_copy));
+            HCG_CUDA(c, cudaStreamWaitEvent(c->st_comp, c->ev_chunk[k], 0));
+            const int rc = hcgrid_accumulate(c, (int64_t)m, c->d_in_lon.as<double>() + lo, c->d_in_lat.as<double>() + lo,
+                                             c->d_in_val.as<float>() + (size_t)lo * nchan, nchan,
+                                             weights ? c->d_in_wgt.as<float>() + lo : nullptr, c->st_comp);
+            if (rc != HCGRID_OK) { cudaDeviceSynchronize(); c->acc_nchan = 0; return rc; }
+        }
+        const int rc = hcgrid_finalize(c, c->d_out_cube.p, c->d_out_w.p, counts ? c->d_out_cnt.as<int32_t>() : nullptr, 1,
+                                       c->st_comp);
+        if (rc != HCGRID_OK) { cudaDeviceSynchronize(); c->acc_nchan = 0; return rc; }
+        HCG_CUDA(c, cudaMemcpyAsync(cube, c->d_out_cube.p, nc * (size_t)nchan * osz, cudaMemcpyDeviceToHost, c->st_comp));
+        HCG_CUDA(c, cudaMemcpyAsync(wmap, c->d_out_w.p, nc * osz, cudaMemcpyDeviceToHost, c->st_comp));
+        if (counts) HCG_CUDA(c, cudaMemcpyAsync(counts, c->d_out_cnt.p, nc * 4, cudaMemcpyDeviceToHost, c->st_comp));
+        HCG_CUDA(c, cudaStreamSynchronize(c->st_comp));
+        c->stats.n_samples = n;
+        return HCGRID_OK;
+    }
     cudaStream_t st = nullptr;   // legacy default stream: ordered with everything
     if (n > 0) {
         HCG_CUDA(c, cudaMemcpyAsync(c->d_in_lon.p, lon, nn * 8, cudaMemcpyHostToDevice, st));

@@ -163,6 +163,9 @@ struct hcgrid_ctx {
     const double* last_lat = nullptr;
     int64_t last_n = 0;
     cudaStream_t last_stream = nullptr;
+    cudaStream_t st_copy = nullptr, st_comp = nullptr;   // hcgrid_grid_host pipeline (created on first use)
+    cudaEvent_t ev_chunk[16] = {};
+    int opt_host_chunks = 0;
     cudaEvent_t ev[8] = {};
     bool ev_valid = false;
     hcgrid_stats stats{};

@@ -655,3 +655,30 @@ def test_row_band_sharding_on_one_gpu(oracle):
         cubes.append(cube.cpu().numpy()); wmaps.append(wmap.cpu().numpy()); cnts.append(cnt.cpu().numpy())
         g.close()
     compare(np.concatenate(cubes), np.concatenate(wmaps), np.concatenate(cnts), ref, w.sigma_deg, w.radius_deg, TOL_F32)
+
+
+@pytest.mark.parametrize("cfg,precision,chunks", [(1, "f32", 3), (3, "f32", 4), (4, "f32", 2), (5, "f32", 5), (2, "f64", 3)])
+def test_host_entry_point_in_chunks(oracle, cfg, precision, chunks):
+    """hcgrid_grid_host with the copy / compute pipeline forced on (HCGRID_OPT_HOST_CHUNKS): pieces gridded as
+    they arrive, one normalisation at the end; pinned and pageable buffers; then the plain path again."""
+    from paper_2012_13173_b200 import binding
+    w, ref = mini(oracle, cfg)
+    g = binding.HCGrid(w.sigma_deg, w.radius_deg, w.nside, precision=precision)
+    t = w.target
+    g.set_target_car(t.nx, t.ny, t.lon0, t.lat0, t.dlon, t.dlat)
+    g.set_option(binding.OPT_HOST_CHUNKS, chunks)
+    tol = TOL_F64 if precision == "f64" else TOL_F32
+    pin = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
+    for conv in (pin, lambda a: a):
+        cube, wmap, cnt = g.grid_host(conv(w.lon), conv(w.lat), conv(w.values), conv(w.weights))
+        compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, tol, qmax(w))
+        assert g.accumulated_batches == 0
+    again = g.grid_host(w.lon, w.lat, w.values, w.weights)
+    assert np.array_equal(again[0], cube, equal_nan=True) and np.array_equal(again[1], wmap)   # deterministic
+    g.set_option(binding.OPT_HOST_CHUNKS, 1)
+    cube1, wmap1, cnt1 = g.grid_host(w.lon, w.lat, w.values, w.weights)
+    compare(cube1, wmap1, cnt1, ref, w.sigma_deg, w.radius_deg, tol, qmax(w))
+    assert np.array_equal(cnt1, cnt)
+    with pytest.raises(binding.HCGridError):
+        g.set_option(binding.OPT_HOST_CHUNKS, 17)
+    g.close()
