@@ -239,7 +239,8 @@ int hcgrid_grid_host(hcgrid_ctx* c, int64_t n, const double* lon, const double* 
         for (int k = 0; k < chunks; ++k)
             if (!c->ev_chunk[k]) HCG_CUDA(c, cudaEventCreateWithFlags(&c->ev_chunk[k], cudaEventDisableTiming));
         HCG_CUDA(c, cudaDeviceSynchronize());               // scratch may still be in use on the caller's streams
-        const int64_t per = ((n + chunks - 1) / chunks + 63) & ~(int64_t)63;   // keeps value rows 16-byte aligned
+        // equal pieces but a last one of half the size: its gridding is what the copy cannot hide
+        const int64_t per = ((int64_t)((double)n / ((double)chunks - 0.5)) + 64) & ~(int64_t)63;   // value rows stay 16-byte aligned
         for (int k = 0; k < chunks; ++k) {
             const int64_t lo = std::min<int64_t>(n, (int64_t)k * per), hi = std::min<int64_t>(n, lo + per);
             const size_t m = (size_t)(hi - lo);
