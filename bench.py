@@ -340,7 +340,8 @@ def run_product(args):
                    "l2": "inputs larger than L2 (no flush): lon/lat/values %.0f MB + packed records %.0f MB per step"
                          % (h2d / 1e6, st["n_kept"] * 16 / 1e6),
                    "coarsen": st["coarsen"], "coarsen_y": st["coarsen_y"], "subpix_bits": st["subpix_bits"],
-                   "preorder": {1: "radix sort", 2: "counting sort"}.get(st["preorder"], "?"), "per_rank": "one independent problem" if units_total is None else "a band of target rows + its samples (rank 0's figures in roofline / stages)",
+                   "preorder": {1: "radix sort", 2: "counting sort"}.get(st["preorder"], "?"),
+                   "e2e_path": "hcgrid_grid_host, pinned buffers; inputs of 64 MB or more are copied in 4 pieces and gridded as they arrive", "per_rank": "one independent problem" if units_total is None else "a band of target rows + its samples (rank 0's figures in roofline / stages)",
                    "outputs": "datacube + weight map (count output off in the timed calls)"},
         "kernel_evals_per_s": n_hit * world * args.steps / (ms_total * 1e-3),
         "conv_kernel": {"us": t_conv * 1e6, "cell_channels_per_s": ncell * nchan / t_conv,
