@@ -15,11 +15,15 @@ namespace hcg {
 static double __longlong_as_double_host(long long v) { double d; std::memcpy(&d, &v, 8); return d; }
 static float __int_as_float_host(int v) { float f; std::memcpy(&f, &v, 4); return f; }
 
+// acc += part for the three outputs of one batch in one launch (thread i: sum i, and cell i's
+// weight and count while i < ncell).
 template <typename T>
 __global__ void __launch_bounds__(256)
-add_sums_kernel(T* __restrict__ acc, const T* __restrict__ part, int64_t n) {
+add_batch_kernel(T* __restrict__ acc_cube, const T* __restrict__ cube, int64_t ne, T* __restrict__ acc_w,
+                 const T* __restrict__ w, int32_t* __restrict__ acc_cnt, const int32_t* __restrict__ cnt, int64_t nc) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) acc[i] += part[i];
+    if (i < ne) acc_cube[i] += cube[i];
+    if (i < nc) { acc_w[i] += w[i]; acc_cnt[i] += cnt[i]; }
 }
 
 template <typename T>
@@ -42,33 +46,34 @@ template <typename T>
 static int accumulate_impl(hcgrid_ctx* c, int64_t n, const double* lon, const double* lat, const float* values,
                            int nchan, const float* weights, cudaStream_t st) {
     const size_t nc = (size_t)c->ncell, ne = nc * (size_t)nchan;
-    HCG_CUDA(c, c->d_tmp_cube.ensure(ne * sizeof(T)));
-    HCG_CUDA(c, c->d_tmp_w.ensure(nc * sizeof(T)));
-    HCG_CUDA(c, c->d_tmp_cnt.ensure(nc * 4));
-    if (c->acc_nchan == 0) {                                // first batch: zeroed accumulators
+    if (c->acc_nchan == 0) {
+        // first batch: its un-normalised sums ARE the accumulators
         HCG_CUDA(c, c->d_acc_cube.ensure(ne * sizeof(T)));
         HCG_CUDA(c, c->d_acc_w.ensure(nc * sizeof(T)));
         HCG_CUDA(c, c->d_acc_cnt.ensure(nc * 4));
-        HCG_CUDA(c, cudaMemsetAsync(c->d_acc_cube.p, 0, ne * sizeof(T), st));
-        HCG_CUDA(c, cudaMemsetAsync(c->d_acc_w.p, 0, nc * sizeof(T), st));
-        HCG_CUDA(c, cudaMemsetAsync(c->d_acc_cnt.p, 0, nc * 4, st));
+        c->raw_sums = true;
+        const int rc = hcgrid_grid(c, n, lon, lat, values, nchan, weights, c->d_acc_cube.p, c->d_acc_w.p,
+                                   c->d_acc_cnt.as<int32_t>(), st);
+        c->raw_sums = false;
+        if (rc != HCGRID_OK) return rc;
         c->acc_nchan = nchan;
-        c->acc_batches = 0;
+        c->acc_batches = 1;
+        return HCGRID_OK;
     }
+    HCG_CUDA(c, c->d_tmp_cube.ensure(ne * sizeof(T)));
+    HCG_CUDA(c, c->d_tmp_w.ensure(nc * sizeof(T)));
+    HCG_CUDA(c, c->d_tmp_cnt.ensure(nc * 4));
     c->raw_sums = true;
     const int rc = hcgrid_grid(c, n, lon, lat, values, nchan, weights, c->d_tmp_cube.p, c->d_tmp_w.p,
                                c->d_tmp_cnt.as<int32_t>(), st);
     c->raw_sums = false;
     if (rc != HCGRID_OK) return rc;
     const int threads = 256;
-    add_sums_kernel<T><<<(unsigned)((ne + threads - 1) / threads), threads, 0, st>>>(c->d_acc_cube.as<T>(),
-                                                                                  c->d_tmp_cube.as<T>(), (int64_t)ne);
-    add_sums_kernel<T><<<(unsigned)((nc + threads - 1) / threads), threads, 0, st>>>(c->d_acc_w.as<T>(),
-                                                                                  c->d_tmp_w.as<T>(), (int64_t)nc);
-    add_sums_kernel<int32_t><<<(unsigned)((nc + threads - 1) / threads), threads, 0, st>>>(
+    add_batch_kernel<T><<<(unsigned)((ne + threads - 1) / threads), threads, 0, st>>>(
+        c->d_acc_cube.as<T>(), c->d_tmp_cube.as<T>(), (int64_t)ne, c->d_acc_w.as<T>(), c->d_tmp_w.as<T>(),
         c->d_acc_cnt.as<int32_t>(), c->d_tmp_cnt.as<int32_t>(), (int64_t)nc);
     HCG_CUDA(c, cudaGetLastError());
-    c->stats.gpu_launches += 3;
+    c->stats.gpu_launches += 1;
     c->acc_batches += 1;
     return HCGRID_OK;
 }

@@ -595,6 +595,12 @@ def test_accumulate_batches_equal_the_union(oracle, cfg, precision):
         compare(cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy(), ref, w.sigma_deg, w.radius_deg, tol, qmax(w))
     with pytest.raises(binding.HCGridError):
         g.finalize()
+    # an EMPTY first batch (it becomes the accumulators), then everything
+    g.accumulate(lon[:0].contiguous(), lat[:0].contiguous(), val[:0].contiguous(), None if wts is None else wts[:0].contiguous())
+    g.accumulate(lon, lat, val, wts)
+    cube, wmap, cnt = g.finalize()
+    torch.cuda.synchronize()
+    compare(cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy(), ref, w.sigma_deg, w.radius_deg, tol, qmax(w))
     g.close()
 
 
