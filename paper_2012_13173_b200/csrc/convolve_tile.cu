@@ -142,15 +142,19 @@ conv1_tile_f32(const TileArgs a) {
         int i = part * 32 + lane;
         stream_seek(min(i, last), tp, end, base);
         uint4 ra = ldg_rec(base, min(i, last));
+        int i1 = i + stride;
+        stream_seek(min(i1, last), tp, end, base);
+        uint4 rn = ldg_rec(base, min(i1, last));
         tc.hm = tc.hmax;
-#pragma unroll 2
+#pragma unroll 3
         for (int it = part; it < nfull; it += S) {
-            i += stride;
-            const int ii = min(i, last);
+            const int i2 = i1 + stride;
+            const int ii = min(i2, last);
             stream_seek(ii, tp, end, base);
-            const uint4 rb = ldg_rec(base, ii);
+            const uint4 rc = ldg_rec(base, ii);
             tile_pairs<GX, GY, MODE, COUNTS, KFN>(ra, tc, W, S_, cnt);
-            ra = rb;
+            ra = rn; rn = rc;
+            i = i1; i1 = i2;
         }
         if ((total & 31) && (nfull & (S - 1)) == part) {  // the ragged last step belongs to one warp
             tc.hm = i <= last ? tc.hmax : -1.0f;
