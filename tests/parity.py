@@ -49,9 +49,14 @@ def compare(cube, wmap, counts, ref, sigma_deg, radius_deg, tol, qmax=1.0, cells
     assert badv.shape[0] == 0, (f"{badv.shape[0]} datacube entries out of tolerance; first: {badv[0]} gpu "
                                 f"{cube[ok][tuple(badv[0])]!r} oracle {ref.datacube[ok][tuple(badv[0])]!r}")
     nz = ref.weightmap > 0
+    clear = nz & (nb == 0)          # cells no boundary pair (reading c4) can move
+    relv = errv / np.maximum(scale, 1e-300)
     return {
         "max_rel_w": float(np.max(errw[nz] / ref.weightmap[nz])) if nz.any() else 0.0,
-        "max_rel_v": float(np.max(errv / np.maximum(scale, 1e-300))) if ok.any() else 0.0,
+        "max_rel_v": float(np.max(relv)) if ok.any() else 0.0,
+        "max_rel_w_clear": float(np.max(errw[clear] / ref.weightmap[clear])) if clear.any() else 0.0,
+        "max_rel_v_clear": float(np.max(relv[(nb == 0)[ok]])) if clear.any() else 0.0,
+        "cells_with_boundary_pairs": int(np.count_nonzero(nb)),
         "near_boundary_pairs": int(nb.sum()),
         "n_hit": int(ref.counts.sum()),
     }
