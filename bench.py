@@ -4,6 +4,10 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl reference]
 
+With --gpus N > 1 and no torchrun environment the script starts the N ranks itself (one process
+per GPU, rendezvous on 127.0.0.1); under torchrun it uses the ranks it was given and fails if
+their number differs from --gpus.
+
 A step is one pass of the whole hot path (a2 pixelise, a3 sort, a4 tables, a5 pack, a6
 convolve: one hcgrid_grid call) over one batch of seeded synthetic input, by default
 BASELINE config 3 ("dense scan", 10 M samples, 1200 x 1200 cells) -- the configuration the
@@ -366,6 +370,35 @@ def run_product(args):
     return 0
 
 
+# ------------------------------------------------------------------------------- N ranks on one node
+def free_port() -> int:
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def child_envs(n: int, port: int, base=None) -> list:
+    """Environment of each of the N ranks `python bench.py --gpus N` starts when it is not already
+    running under torchrun: one process per GPU, rendezvous on 127.0.0.1 (the container hostname
+    may not resolve)."""
+    base = dict(os.environ if base is None else base)
+    return [dict(base, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE=str(n), LOCAL_WORLD_SIZE=str(n),
+                 MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port)) for r in range(n)]
+
+
+def launch_ranks(n: int, argv: list) -> int:
+    """Start N copies of this script, one per GPU; rank 0 prints the JSON line.  NCCL's own log
+    (NCCL_DEBUG) is passed through untouched."""
+    procs = [subprocess.Popen([sys.executable, os.path.abspath(__file__), *argv], env=env)
+             for env in child_envs(n, free_port())]
+    rcs = [p.wait() for p in procs]
+    bad = [(r, rc) for r, rc in enumerate(rcs) if rc != 0]
+    if bad:
+        sys.stderr.write(f"bench.py: ranks failed (rank, exit code): {bad}\n")
+    return max(abs(rc) for rc in rcs)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -382,6 +415,13 @@ def main():
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per launch of the convolution kernel from the committed ncu capture")
     args = ap.parse_args()
+    if args.gpus < 1:
+        raise SystemExit("bench.py: --gpus must be >= 1")
+    world = os.environ.get("WORLD_SIZE")
+    if world is None and args.gpus > 1:
+        return launch_ranks(args.gpus, sys.argv[1:])       # not under torchrun: start the N ranks here
+    if world is not None and int(world) != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but the launcher started WORLD_SIZE={world} ranks")
     if args.impl == "reference":
         return run_reference(args)
     return run_product(args)

@@ -31,3 +31,36 @@ def test_reference_arm_other_ranks_exit_quietly():
                         "--config", "1", "--steps", "1", "--warmup", "0"], capture_output=True, text=True, timeout=600,
                        cwd=ROOT, env=env)
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def test_gpus_n_without_torchrun_starts_n_ranks_and_prints_one_line():
+    """`python bench.py --gpus 2` with no launcher environment must start the 2 ranks itself
+    (SURVEY.md 8e); the reference arm needs no GPU, so the whole launch path runs here."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
+                        "--config", "1", "--steps", "1", "--warmup", "0"], capture_output=True, text=True, timeout=600,
+                       cwd=ROOT, env=env)
+    assert r.returncode == 0, r.stderr
+    lines = [ln for ln in r.stdout.splitlines() if ln.strip()]
+    assert len(lines) == 1, r.stdout
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["impl"] == "reference"
+
+
+def test_launcher_builds_one_environment_per_rank():
+    sys.path.insert(0, ROOT)
+    import bench
+    envs = bench.child_envs(4, 29512, base={"PATH": "/bin", "NCCL_DEBUG": "INFO"})
+    assert len(envs) == 4
+    for r, e in enumerate(envs):
+        assert e["RANK"] == str(r) and e["LOCAL_RANK"] == str(r) and e["WORLD_SIZE"] == "4"
+        assert e["MASTER_ADDR"] == "127.0.0.1" and e["MASTER_PORT"] == "29512"
+        assert e["NCCL_DEBUG"] == "INFO"                      # the communicator's log is not silenced
+
+
+def test_rank_count_mismatch_fails_loudly():
+    env = dict(os.environ, RANK="0", WORLD_SIZE="2", LOCAL_RANK="0")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "4",
+                        "--config", "1", "--steps", "1", "--warmup", "0"], capture_output=True, text=True, timeout=120,
+                       cwd=ROOT, env=env)
+    assert r.returncode != 0 and "WORLD_SIZE=2" in r.stderr
