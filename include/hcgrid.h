@@ -65,7 +65,8 @@ enum {
                                     3 = force the general (any nchan) kernel with fp32 pair arithmetic;
                                     4 = force the TMA-staged single-channel kernel;
                                     5 = force the tile kernel (error if the target does not allow it);
-                                    6 = force the cube kernel (nchan > 1; error if not applicable) */
+                                    6 = force the CUDA-core cube kernel (nchan > 1; error if not applicable);
+                                    7 = force the tensor-core cube kernel (tcgen05; nchan a multiple of 32) */
     HCGRID_OPT_WARPS_PER_SM = 5, /* resident convolution warps per SM (staged kernel); 0 = auto */
     HCGRID_OPT_COARSEN_Y = 6,    /* target rows per warp task (tile kernel); 0 = auto */
     HCGRID_OPT_SPLIT = 7,        /* warps sharing one tile's candidate stream (tile kernel): 1, 2, 4; 0 = auto */

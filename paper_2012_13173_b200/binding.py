@@ -21,7 +21,7 @@ F32, F64 = 0, 1
 OPT_PROFILE, OPT_SUBPIX_BITS, OPT_COARSEN, OPT_KERNEL, OPT_WARPS_PER_SM, OPT_COARSEN_Y, OPT_SPLIT, OPT_PREORDER = 1, 2, 3, 4, 5, 6, 7, 8
 OPT_HOST_CHUNKS = 9
 PREORDER_AUTO, PREORDER_RADIX, PREORDER_COUNTING = 0, 1, 2
-KERNEL_AUTO, KERNEL_SIMPLE, KERNEL_F64PAIR, KERNEL_GENERAL, KERNEL_STAGED, KERNEL_TILE, KERNEL_CUBE = 0, 1, 2, 3, 4, 5, 6
+KERNEL_AUTO, KERNEL_SIMPLE, KERNEL_F64PAIR, KERNEL_GENERAL, KERNEL_STAGED, KERNEL_TILE, KERNEL_CUBE, KERNEL_CUBE_TC = 0, 1, 2, 3, 4, 5, 6, 7
 
 EXPORTS = [
     "hcgrid_create", "hcgrid_destroy", "hcgrid_set_option", "hcgrid_set_target_car",

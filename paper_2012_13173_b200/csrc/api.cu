@@ -85,7 +85,7 @@ int hcgrid_destroy(hcgrid_ctx* c) {
     if (!c) return HCGRID_OK;
     cudaSetDevice(c->device);
     DevBuf* bufs[] = {&c->d_strips, &c->d_wins, &c->d_winsf, &c->d_rowsf, &c->d_cell_lon, &c->d_cell_lat, &c->d_keys, &c->d_keys_out,
-                      &c->d_idx, &c->d_idx_out, &c->d_sort_tmp, &c->d_bins, &c->d_rec, &c->d_misc, &c->d_long,
+                      &c->d_idx, &c->d_idx_out, &c->d_sort_tmp, &c->d_bins, &c->d_rec, &c->d_misc, &c->d_long, &c->d_dirty,
                       &c->d_in_lon, &c->d_in_lat, &c->d_in_val, &c->d_in_wgt, &c->d_out_cube, &c->d_out_w,
                       &c->d_out_cnt, &c->d_acc_cube, &c->d_acc_w, &c->d_acc_cnt, &c->d_tmp_cube, &c->d_tmp_w,
                       &c->d_tmp_cnt};
@@ -111,7 +111,7 @@ int hcgrid_set_option(hcgrid_ctx* c, int option, int64_t value) {
             c->opt_coarsen = (int)value;
             break;
         case HCGRID_OPT_KERNEL:
-            if (value < 0 || value > 6) return fail(c, HCGRID_ERR_INVALID_ARG, "kernel must be 0..6");
+            if (value < 0 || value > 7) return fail(c, HCGRID_ERR_INVALID_ARG, "kernel must be 0..7");
             c->opt_kernel = (int)value;
             break;
         case HCGRID_OPT_COARSEN_Y:

@@ -327,11 +327,28 @@ int run_convolve(hcgrid_ctx* c, int64_t n, const float* values, int nchan, bool 
     if (c->opt_kernel == 5 && !(f32 && nchan == 1 && c->tile_ok))
         return fail(c, HCGRID_ERR_UNSUPPORTED, "the tile kernel needs fp32 mode, one channel and a plate-carree "
                     "target whose reach is a plain longitude window");
-    const bool mc_ok = f32 && nchan > 1 && c->tile_ok && nchan % 4 == 0 && ((uintptr_t)values & 15) == 0;
+    const bool mc_ok = f32 && nchan > 1 && c->tile_ok && nchan % 4 == 0 && ((uintptr_t)values & 15) == 0 &&
+                       ((uintptr_t)cube & 15) == 0;
     if (c->opt_kernel == 6 && !mc_ok)
         return fail(c, HCGRID_ERR_UNSUPPORTED, "the cube kernel needs fp32 mode, nchan a multiple of 4 (> 1), 16-byte "
-                    "aligned values and a plate-carree target whose reach is a plain longitude window");
-    if (mc_ok && (c->opt_kernel == 0 || c->opt_kernel == 6)) {
+                    "aligned values and datacube and a plate-carree target whose reach is a plain longitude window");
+    // tensor-core cube kernel: channel blocks the MMA shapes allow (N a multiple of 32)
+    const bool tc_ok = mc_ok && nchan % 32 == 0;
+    if (c->opt_kernel == 7 && !tc_ok)
+        return fail(c, HCGRID_ERR_UNSUPPORTED, "the tensor-core cube kernel needs what the cube kernel needs and nchan a "
+                    "multiple of 32");
+    if (tc_ok && (c->opt_kernel == 7 || (c->opt_kernel == 0 && nchan >= 64))) {
+        const size_t nd = (size_t)mc_tc_tiles(c) * (size_t)((nchan + 255) / 256);
+        HCG_CUDA(c, c->d_dirty.ensure(nd * 4));
+        rc = launch_conv_mc_tc(c, values, nchan, (float*)cube, (float*)wmap, counts, c->d_dirty.as<int32_t>(), st);
+        // tiles that met a non-finite value (0 * inf would poison all their cells) are redone cell by cell
+        if (rc == HCGRID_OK) {
+            a.counts = counts;
+            rc = launch_conv_general(c, a, false, false, st, c->d_dirty.as<int32_t>());
+        }
+        c->stats.kernel = 8;
+        if (rc == HCGRID_OK) c->stats.gpu_launches += 1;
+    } else if (mc_ok && (c->opt_kernel == 0 || c->opt_kernel == 6)) {
         rc = launch_conv_mc(c, values, nchan, (float*)cube, (float*)wmap, counts, st);
         c->stats.kernel = 7;
     } else if (f32 && nchan == 1 && c->tile_ok && (c->opt_kernel == 0 || c->opt_kernel == 5)) {

@@ -92,6 +92,12 @@ conv_general(const ConvArgs a) {
     if (task >= a.ntasks) return;
     const int s = (int)(task / a.strip_cells);
     const int ix = (int)(task % a.strip_cells);
+    if (a.dirty) {                                              // warp-uniform
+        const int t16 = (s >> 3) * a.dirty_tiles_x + (ix >> 4);
+        int any = 0;
+        for (int b = 0; b < a.dirty_nblk; ++b) any |= __ldg(a.dirty + (size_t)b * a.dirty_ntiles + t16);
+        if (!any) return;
+    }
     const Strip st = a.strips[s];
     const int nchan = a.nchan;
     const float* __restrict__ values = a.values;
@@ -207,8 +213,13 @@ conv_general(const ConvArgs a) {
     }
 }
 
-int launch_conv_general(hcgrid_ctx* c, const ConvArgs& a0, bool pair_f64, bool out_double, cudaStream_t st) {
+int launch_conv_general(hcgrid_ctx* c, const ConvArgs& a0, bool pair_f64, bool out_double, cudaStream_t st,
+                        const int32_t* dirty) {
     ConvArgs a = a0;
+    a.dirty = dirty;
+    a.dirty_tiles_x = (c->strip_cells + 15) / 16;
+    a.dirty_ntiles = mc_tc_tiles(c);
+    a.dirty_nblk = (a.nchan + 255) / 256;
     a.ntasks = c->ncell;
     a.tasks_per_strip = a.strip_cells;
     const bool vec4 = (a.nchan % 4 == 0) && ((uintptr_t)a.values % 16 == 0);

@@ -151,7 +151,7 @@ struct hcgrid_ctx {
     double dlmax = 0.0;                  // widest longitude half-window of a support disc, rad
     bool tile_ok = false;                // the tile kernel's preconditions hold for this target
     // per-call scratch
-    hcg::DevBuf d_keys, d_keys_out, d_idx, d_idx_out, d_sort_tmp, d_bins, d_rec, d_misc, d_long;
+    hcg::DevBuf d_keys, d_keys_out, d_idx, d_idx_out, d_sort_tmp, d_bins, d_rec, d_misc, d_long, d_dirty;
     hcg::DevBuf d_in_lon, d_in_lat, d_in_val, d_in_wgt, d_out_cube, d_out_w, d_out_cnt;  // *_host path
     // incremental gridding (hcgrid_accumulate / hcgrid_finalize): un-normalised sums over the batches so far
     hcg::DevBuf d_acc_cube, d_acc_w, d_acc_cnt, d_tmp_cube, d_tmp_w, d_tmp_cnt;

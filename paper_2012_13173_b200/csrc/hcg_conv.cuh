@@ -25,6 +25,10 @@ struct ConvArgs {
     int32_t small64;            // 1: fp64 pairs by the small-angle series (pair64_small), 0: full functions
     float qx, qy;               // radians per fixed-point unit
     double sx;                  // fixed-point units per radian (lon)
+    // fix-up pass of the general kernel after the tensor-core cube kernel (convolve_mc_tc.cu): only the cells of
+    // the 16 x 8-cell tiles flagged in dirty[blk * dirty_ntiles + tile] are recomputed (nullptr: every cell)
+    const int32_t* dirty;
+    int32_t dirty_tiles_x, dirty_ntiles, dirty_nblk;
 };
 
 __device__ __forceinline__ float ex2_approx(float x) {
@@ -99,7 +103,14 @@ int launch_conv_tile(hcgrid_ctx* c, int64_t n, float* cube, float* wmap, int32_t
 int launch_conv_mc(hcgrid_ctx* c, const float* values, int nchan, float* cube, float* wmap, int32_t* counts,
                    cudaStream_t st);
 
-// launcher of convolve_gen.cu
-int launch_conv_general(hcgrid_ctx* c, const ConvArgs& a, bool pair_f64, bool out_double, cudaStream_t st);
+// launcher of convolve_mc_tc.cu (tcgen05 / TMEM; many channels, fp32, plate-carree targets, nchan % 32 == 0);
+// dirty [ceil(nchan / 256)][mc_tc_tiles] receives 1 for every tile that met a non-finite value
+int launch_conv_mc_tc(hcgrid_ctx* c, const float* values, int nchan, float* cube, float* wmap, int32_t* counts,
+                      int32_t* dirty, cudaStream_t st);
+int mc_tc_tiles(const hcgrid_ctx* c);
+
+// launcher of convolve_gen.cu; dirty: see ConvArgs
+int launch_conv_general(hcgrid_ctx* c, const ConvArgs& a, bool pair_f64, bool out_double, cudaStream_t st,
+                        const int32_t* dirty = nullptr);
 
 }  // namespace hcg

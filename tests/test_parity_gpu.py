@@ -151,10 +151,10 @@ def test_cube_kernel_channel_counts(oracle, nchan):
     w.weights = rng.uniform(0.5, 1.5, n).astype(np.float32)
     w.target = workloads.CarTarget(23, 19, 29.8, 19.85, 1.0 / 60.0, 1.0 / 60.0)
     ref = run_oracle(oracle, w)
-    cube, wmap, cnt, st = run_gpu(w, "f32")
+    cube, wmap, cnt, st = run_gpu(w, "f32", {binding.OPT_KERNEL: 6})
     assert st["kernel"] == 7
     compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F32, qmax(w))
-    cube, wmap, cnt, st = run_gpu(w, "f32", want_counts=False)
+    cube, wmap, cnt, st = run_gpu(w, "f32", {binding.OPT_KERNEL: 6}, want_counts=False)
     compare(cube, wmap, None, ref, w.sigma_deg, w.radius_deg, TOL_F32, qmax(w))
     cube, wmap, cnt, st = run_gpu(w, "f32", {binding.OPT_KERNEL: binding.KERNEL_GENERAL})
     assert st["kernel"] == 3
@@ -170,7 +170,7 @@ def test_cube_kernel_falls_back_for_odd_channel_counts(oracle):
     assert st["kernel"] == 3
     compare(cube, wmap, cnt, ref2, w2.sigma_deg, w2.radius_deg, TOL_F32)
     _, _, _, st = run_gpu(w, "f32")
-    assert st["kernel"] == 7
+    assert st["kernel"] == 8                     # 256 channels: the tensor-core cube kernel
 
 
 @pytest.mark.parametrize("radius_deg,sigma_deg", [(0.1, 0.04), (0.2, 0.08), (1.5, 0.5)])
