@@ -6,26 +6,29 @@
 // For a tile of 128 target cells the weighted sums are a matrix product
 //     S[cell][chan] = sum_k  A[cell][k] * B[k][chan],   A = q_k w(d(cell, k)),  B = spectrum of candidate k,
 // over the K candidates that can reach the tile.  One CTA owns a tile of 16 x 8 cells (M = 128) and a
-// block of up to 256 channels (N):
-//   * one warp builds the candidate stream of the tile (ring table, lookup-bin windows: steps i-iii, as
-//     in convolve_tile.cu) and keeps the candidates whose distance to the tile's rectangle of cell
-//     centres is within R: compaction in stream order into a FIFO of 16-candidate groups, each entry
-//     with a 4-bit mask of the 8 x 4-cell quarters of the tile the candidate can reach;
-//   * 8 compute warps evaluate A per stage (= group) of 16 candidates: thread = cell, a warp = one
-//     quarter of the tile, which visits only the candidates that can reach it, two at a time; the tile
-//     kernel's fp32 pair arithmetic on exact fixed-point differences; every weight is split
-//     w = hi + lo (hi = w rounded to TF32) and both go to the UMMA K-major core-matrix layout;
-//   * 2 warps copy the candidates' spectrum rows IN PLACE from `values` (never moved: a5) with cp.async
-//     into the UMMA MN-major SWIZZLE_128B_BASE32B layout, two stages ahead, and write
+// block of up to 256 channels (N); its warps are specialised:
+//   * stream warp: builds the candidate stream of the tile (ring table, lookup-bin windows: steps i-iii,
+//     as in convolve_tile.cu) and keeps the candidates whose distance to the tile's rectangle of cell
+//     centres is within R: compaction in stream order into a FIFO of 32-candidate groups (= pipeline
+//     stages).  A candidate's fixed-point offset from the tile centre is stored as two floats each
+//     (multiple of 4096 + remainder, both exact), so the cell - candidate differences are formed with
+//     three fp32 additions and carry the same single rounding as the tile kernel's integer difference;
+//   * 8 compute warps evaluate A: thread = cell (= MMA row = TMEM lane), all 16 candidates of its two
+//     K-steps of a stage, two candidates per instruction (packed fma.rn.f32x2 / add / mul), with the
+//     tile kernel's scaled pair arithmetic; every weight is split w = hi + lo (hi = w rounded to TF32)
+//     and stored straight into TENSOR MEMORY (tcgen05.st), from where the MMA reads its A operand -- no
+//     shared-memory round trip and no proxy fence on this path;
+//   * 4 spectrum-row warps copy the candidates' spectrum rows IN PLACE from `values` (never moved: a5)
+//     with cp.async into the UMMA MN-major SWIZZLE_128B_BASE32B layout, a stage ahead, and write
 //     lo = v - trunc_tf32(v) beside them (the tensor core itself ignores the low 13 bits of v);
-//   * one thread issues, per 8 candidates, three tcgen05.mma.kind::tf32 (hi*v, lo*v, hi*lo_v: 3xTF32,
-//     product error <= ~3e-6 relative) into a 128 x 256 fp32 accumulator in TMEM;
-//   * the tensor core adds with round-toward-zero (measured: -3.4e-8 relative per update), so the
-//     TMEM accumulator only ever holds a CHUNK of 8 stages (48 updates) -- two accumulators alternate,
-//     and the compute warps add every finished chunk into fp32 registers (round-to-nearest, 128
-//     channels x 1 cell per thread), which also makes the epilogue a plain divide and store.
-// W and the counts are summed on the CUDA cores from the same weights.  No atomics in the sums; the
-// order of the additions is fixed by the stream order, so results are bit-wise reproducible.
+//   * MMA warp: one thread issues, per 8 candidates, three tcgen05.mma.kind::tf32 (hi*v, lo*v, hi*lo_v:
+//     3xTF32, product error <= ~3e-6 relative) into a 128 x 256 fp32 accumulator in TMEM.
+// The tensor core adds with round-toward-zero (measured: -3.4e-8 relative per update), so the TMEM
+// accumulator only ever holds a CHUNK of 4 stages (48 updates): the compute warps add every finished
+// chunk into fp32 registers (round-to-nearest, 128 channels x 1 cell per thread), which also makes the
+// epilogue a plain divide and store.  W and the counts are summed on the CUDA cores from the same
+// weights.  No atomics in the sums; the order of the additions is fixed by the stream order, so results
+// are bit-wise reproducible.
 // Odd tile rows walk the rings south to north, so vertically adjacent tiles, which run at the same
 // time, meet the spectrum rows they share at about the same time (L2 instead of HBM).
 // A non-finite value would poison a whole tile through 0 * inf; tiles whose sums came out non-finite
@@ -42,26 +45,35 @@ struct McTcArgs {
 };
 
 constexpr int kTcTX = 16, kTcTY = 8;           // tile = 128 cells = MMA M
-constexpr int kTcCW = 8;                       // compute warps
+constexpr int kTcCW = 8;                       // compute warps (warps 0 .. 7)
 constexpr int kTcCT = kTcCW * 32;              // compute threads
-constexpr int kTcThreads = kTcCT + 128;        // + the service warpgroup: MMA issuer, stream builder, two spectrum-row warps
-constexpr int kTcBW = 2;                       // spectrum-row (B) warps
-constexpr int kTcNS = 4;                       // pipeline stages
-constexpr int kTcP = 2;                        // stages the spectrum rows are requested ahead
-constexpr int kTcCH = 8;                       // stages per TMEM accumulator chunk
-constexpr int kTcGroups = 64;                  // FIFO: groups of 16 candidates (one group = one stage)
-constexpr int kTcFifo = kTcGroups * 16;
+constexpr int kTcBW = 4;                       // spectrum-row warps (warps 8 .. 11)
+constexpr int kTcThreads = kTcCT + 32 * kTcBW + 128;   // + the service warpgroup: MMA issuer, stream builder, two idle warps
+constexpr int kTcKS = 4;                       // K-steps (of 8 candidates) per pipeline stage
+constexpr int kTcSC = 8 * kTcKS;               // candidates per stage = per FIFO group
+constexpr int kTcNS = 3;                       // pipeline stages (B in shared memory, A in tensor memory)
+constexpr int kTcBD = 1;                       // stages the spectrum rows are requested ahead of their split
+constexpr int kTcCH = 4;                       // stages per TMEM accumulator chunk (3 kTcKS kTcCH updates)
+constexpr int kTcGroups = 16;                  // FIFO groups
+constexpr int kTcFifo = kTcGroups * kTcSC;     // FIFO entries
 constexpr int kTcRings = 128;                  // ring-table entries per pass
-constexpr int kOffAhi = 0, kOffAlo = 8192, kOffBraw = 16384, kOffBlo = 32768, kStageBytes = 49152;
-constexpr int kOffFifoC = kTcNS * kStageBytes;             // uint4 [kTcFifo]: xi, yi, cos(lat_s), q
-constexpr int kOffFifoI = kOffFifoC + kTcFifo * 16;        // uint32 [kTcFifo]: sample index
-constexpr int kOffFifoM = kOffFifoI + kTcFifo * 4;         // uint8 [kTcFifo]: quarters of the tile within reach
-constexpr int kOffTabBase = kOffFifoM + kTcFifo;           // u64 [kTcRings]
+constexpr int kBrawBytes = kTcKS * 8192;       // spectrum rows of a stage: kTcKS K-steps x 8 rows x 1 KB
+constexpr int kOffBraw = 0, kOffBlo = kBrawBytes, kStageBytes = 2 * kBrawBytes;
+constexpr int kTmemA = 256;                    // TMEM columns: accumulator 0 .. 255, A ring from 256
+constexpr int kTmemAStage = 16 * kTcKS;        // per stage: hi kTcKS x 8 columns, then lo kTcKS x 8 columns
+static_assert(kTmemA + kTcNS * kTmemAStage <= 512, "TMEM columns");
+// FIFO: per pair of candidates three float4: (Xh_a, Xh_b, Xl_a, Xl_b), (Yh_a, Yh_b, Yl_a, Yl_b), (cs_a, cs_b, q_a, q_b)
+constexpr int kOffFifoX = kTcNS * kStageBytes;
+constexpr int kOffFifoY = kOffFifoX + kTcFifo * 8;
+constexpr int kOffFifoC = kOffFifoY + kTcFifo * 8;
+constexpr int kOffFifoI = kOffFifoC + kTcFifo * 8;         // uint32 [kTcFifo]: sample index
+constexpr int kOffTabBase = kOffFifoI + kTcFifo * 4;       // u64 [kTcRings]
 constexpr int kOffTabEnd = kOffTabBase + kTcRings * 8;     // int [kTcRings]
 constexpr int kOffGrpN = kOffTabEnd + kTcRings * 4;        // uint32 [kTcGroups]: candidates in the group | 0x80 (last group of the tile)
-constexpr int kOffBars = kOffGrpN + kTcGroups * 4;         // u64: full[NS], empty[NS], dfull[2], dempty[2], cfull[G], cempty[G]
-constexpr int kOffMisc = kOffBars + 8 * (2 * kTcNS + 4 + 2 * kTcGroups);
+constexpr int kOffBars = kOffGrpN + kTcGroups * 4;         // u64: afull[NS], bfull[NS], empty[NS], dfull, dempty, cfull[G], cempty[G]
+constexpr int kOffMisc = kOffBars + 8 * (3 * kTcNS + 2 + 2 * kTcGroups);
 constexpr int kTcSmem = kOffMisc + 64;
+static_assert(kTcSmem <= 227 * 1024, "shared memory");
 
 // ---- PTX wrappers
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -71,13 +83,14 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 // Bounded: a wait that outlasts any legitimate one (seconds) is a broken pipeline -- fail loudly, do not hang.
+// The suspend-time hint keeps a waiting warp off the issue slots of the working ones (it still wakes when the phase completes).
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     for (uint32_t spins = 0;; ++spins) {
         uint32_t ok;
-        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(bar), "r"(parity), "r"(20000u) : "memory");
         if (ok) return;
-        if (spins > (1u << 22)) __trap();
+        if (spins > (1u << 20)) __trap();
     }
 }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -98,6 +111,13 @@ __device__ __forceinline__ void tmem_ld32(uint32_t addr, uint32_t (&v)[32]) {
                    "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
                    "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
                    "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+                 : "r"(addr) : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t addr, uint32_t (&v)[16]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+                 "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
                  : "r"(addr) : "memory");
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
@@ -126,8 +146,60 @@ __device__ __forceinline__ uint32_t lds_u1(uint32_t addr) {
 __device__ __forceinline__ void sts_u4(uint32_t addr, uint4 v) {
     asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
+#ifdef HCG_TC_PROF
+#define PROF_DECL(n) long long prof_[n] = {}; long long prof_t_ = clock64(); const long long prof_t0_ = prof_t_; (void)prof_t0_
+#define PROF_LAP(i) do { const long long t_ = clock64(); prof_[i] += t_ - prof_t_; prof_t_ = t_; } while (0)
+#define PROF_ON (blockIdx.x == 300 && blockIdx.y == 0 && lane == 0)
+#else
+#define PROF_DECL(n)
+#define PROF_LAP(i)
+#endif
 // keep a loop-invariant value in its register (ptxas otherwise recomputes it from the thread index every iteration)
 #define HCG_PIN(x) asm volatile("" : "+r"(x))
+
+__device__ __forceinline__ void umma_tf32_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}"
+                 ::"r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
+}
+__device__ __forceinline__ void tmem_st1(uint32_t addr, float v) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" ::"r"(addr), "f"(v) : "memory");
+}
+__device__ __forceinline__ void tmem_st16_zero(uint32_t addr) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1};"
+                 ::"r"(addr), "r"(0u) : "memory");
+}
+__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+__device__ __forceinline__ unsigned long long f2_pack(float lo, float hi) {
+    unsigned long long d;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi));
+    return d;
+}
+__device__ __forceinline__ void f2_unpack(unsigned long long v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ unsigned long long f2_add(unsigned long long a, unsigned long long b) {
+    unsigned long long d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ unsigned long long f2_mul(unsigned long long a, unsigned long long b) {
+    unsigned long long d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ unsigned long long f2_fma(unsigned long long a, unsigned long long b, unsigned long long c) {
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
+}
 
 // UMMA shared-memory matrix descriptor: start address, leading / stride byte offsets (all >> 4), version 1,
 // layout type (0: no swizzle, 1: SWIZZLE_128B_BASE32B -- the only MN-major layout of 32-bit operands)
@@ -147,8 +219,9 @@ conv_mc_tc_f32(const McTcArgs m) {
     extern __shared__ __align__(1024) unsigned char s_tc[];
     const uint32_t s_base = smem_addr(s_tc);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const uint32_t b_full = s_base + kOffBars, b_empty = b_full + 8 * kTcNS, b_dfull = b_empty + 8 * kTcNS, b_dempty = b_dfull + 16;
-    const uint32_t b_cfull = b_dempty + 16, b_cempty = b_cfull + 8 * kTcGroups;
+    const uint32_t b_afull = s_base + kOffBars, b_bfull = b_afull + 8 * kTcNS, b_empty = b_bfull + 8 * kTcNS;
+    const uint32_t b_dfull = b_empty + 8 * kTcNS, b_dempty = b_dfull + 8;
+    const uint32_t b_cfull = b_dempty + 8, b_cempty = b_cfull + 8 * kTcGroups;
     volatile uint32_t* s_flag = (volatile uint32_t*)(s_tc + kOffMisc);   // [NS] stage flags
     uint32_t* s_tmem = (uint32_t*)(s_tc + kOffMisc + 4 * kTcNS);
     int* s_bad = (int*)(s_tmem + 1);
@@ -161,13 +234,21 @@ conv_mc_tc_f32(const McTcArgs m) {
     const int row0 = ty * kTcTY;
     const int ncols = min(kTcTX, a.nx - ix0);
     const int nrows = min(kTcTY, a.ny - row0);
+    constexpr int kMmaWarp = kTcCW + kTcBW, kStreamWarp = kMmaWarp + 1;
+    // everything is measured from a cell in the middle of the tile (the fixed-point differences are good for +- 8
+    // columns / rows plus the support radius: target.cu)
+    const int ic = ncols >> 1, jc = nrows >> 1;
+    const uint32_t xc0 = (uint32_t)(unsigned long long)__double2ll_rn((a.u0 + (double)(ix0 + ic) * a.du) * a.sx);
+    const uint32_t yc0 = (uint32_t)__ldg((const int*)(a.rows + row0 + jc));
 
-    if (warp == kTcCW) {
+    if (warp == kMmaWarp) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_addr(s_tmem)), "r"(512u));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::);
         if (lane == 0) {
-            for (int s = 0; s < kTcNS; ++s) { mbar_init(b_full + 8 * s, kTcCW + kTcBW); mbar_init(b_empty + 8 * s, 1); }
-            for (int b = 0; b < 2; ++b) { mbar_init(b_dfull + 8 * b, 1); mbar_init(b_dempty + 8 * b, kTcCW); }
+            for (int s = 0; s < kTcNS; ++s) {
+                mbar_init(b_afull + 8 * s, kTcCW); mbar_init(b_bfull + 8 * s, kTcBW); mbar_init(b_empty + 8 * s, 1);
+            }
+            mbar_init(b_dfull, 1); mbar_init(b_dempty, kTcCW);
             for (int j = 0; j < kTcGroups; ++j) { mbar_init(b_cfull + 8 * j, 1); mbar_init(b_cempty + 8 * j, kTcCW + kTcBW); }
             *s_bad = 0;
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -178,54 +259,61 @@ conv_mc_tc_f32(const McTcArgs m) {
     tc_fence_after();
     const uint32_t tm = *s_tmem;
 
-    if (warp >= kTcCW) {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");       // the whole service warpgroup, one instruction
-        if (warp == kTcCW) {
+    if (warp >= kMmaWarp) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");       // the whole service warpgroup, one instruction
+        if (warp == kMmaWarp) {
             // ============================================================ MMA issuer (lane 0 issues; the warp stays converged)
             const uint32_t idesc = umma_idesc_tf32(nch);
-            const uint64_t a_hi0 = umma_desc(s_base + kOffAhi, 2048, 128, 0), a_lo0 = umma_desc(s_base + kOffAlo, 2048, 128, 0);
             const uint64_t b_rw0 = umma_desc(s_base + kOffBraw, 1024, 512, 1), b_lo0 = umma_desc(s_base + kOffBlo, 1024, 512, 1);
+            PROF_DECL(4);
             for (int s = 0;; ++s) {
                 const int slot = s % kTcNS;
-                mbar_wait(b_full + 8 * slot, (uint32_t)(s / kTcNS) & 1u);
+                const uint32_t par = (uint32_t)(s / kTcNS) & 1u;
+                PROF_LAP(0);
+                mbar_wait(b_afull + 8 * slot, par);
+                PROF_LAP(1);
                 const uint32_t flag = s_flag[slot];
-                tc_fence_after();
                 if (!(flag & 2u)) {
-                    const int chunk = s / kTcCH, buf = chunk & 1;
+                    mbar_wait(b_bfull + 8 * slot, par);
+                    PROF_LAP(2);
+                    const int chunk = s / kTcCH;
                     const bool first = s % kTcCH == 0;
-                    if (first && chunk >= 2) {
-                        mbar_wait(b_dempty + 8 * buf, (uint32_t)((chunk >> 1) - 1) & 1u);
-                        tc_fence_after();
-                    }
+                    if (first && chunk >= 1) mbar_wait(b_dempty, (uint32_t)(chunk - 1) & 1u);   // the previous chunk has been taken over
+                    PROF_LAP(3);
+                    tc_fence_after();
                     if (lane == 0) {
-                        const uint32_t d = tm + (uint32_t)buf * 256u;
                         const uint64_t so = (uint64_t)((uint32_t)slot * (kStageBytes >> 4));
 #pragma unroll
-                        for (int ks = 0; ks < 2; ++ks) {
-                            const uint64_t ah = a_hi0 + so + (uint64_t)(ks * (4096 >> 4)), al = a_lo0 + so + (uint64_t)(ks * (4096 >> 4));
+                        for (int ks = 0; ks < kTcKS; ++ks) {
+                            const uint32_t ah = tm + kTmemA + (uint32_t)(slot * kTmemAStage + ks * 8), al = ah + 8 * kTcKS;
                             const uint64_t br = b_rw0 + so + (uint64_t)(ks * (8192 >> 4)), bl = b_lo0 + so + (uint64_t)(ks * (8192 >> 4));
-                            umma_tf32(d, ah, br, idesc, (first && ks == 0) ? 0u : 1u);
-                            umma_tf32(d, al, br, idesc, 1u);
-                            umma_tf32(d, ah, bl, idesc, 1u);
+#ifndef HCG_TC_NOMMA
+                            umma_tf32_ts(tm, ah, br, idesc, (first && ks == 0) ? 0u : 1u);
+                            umma_tf32_ts(tm, al, br, idesc, 1u);
+                            umma_tf32_ts(tm, ah, bl, idesc, 1u);
+#else
+                            (void)ah; (void)al; (void)br; (void)bl;
+#endif
                         }
                         tc_commit(b_empty + 8 * slot);
-                        if (s % kTcCH == kTcCH - 1 || (flag & 1u)) tc_commit(b_dfull + 8 * buf);
+                        if (s % kTcCH == kTcCH - 1 || (flag & 1u)) tc_commit(b_dfull);
                     }
                     __syncwarp();
                 }
-                if (flag & 1u) break;
+                if (flag & 1u) {
+#ifdef HCG_TC_PROF
+                    if (PROF_ON) printf("MMA: stages %d total %lld | issue+misc %lld wait_afull %lld wait_bfull %lld wait_dempty %lld\n", s + 1, clock64() - prof_t0_, prof_[0], prof_[1], prof_[2], prof_[3]);
+#endif
+                    break;
+                }
             }
-        } else if (warp == kTcCW + 1) {
+        } else if (warp == kStreamWarp) {
             // ============================================================ stream builder: steps (i)-(iii) + compaction
-            // Everything relative to a cell in the middle of the tile (the fixed-point differences are good for +- 8
-            // columns / rows plus the support radius: target.cu).
-            uint32_t xc0 = 0, yc0 = 0;
             float cc0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f, ccmin = 2.0f;
-            float bxlo[2], bxhi[2], bylo[2], byhi[2];                // extents of the cell centres of the four 8 x 4 quarters
+            float xlo, xhi, ylo, yhi;                                // extent of the tile's cell centres (scaled units)
             int rmin = 0x7fffffff, rmax = -0x7fffffff;
             const float sxk = a.sxk, syk = a.syk, a12 = a.a12;
             {
-                const int ic = ncols >> 1, jc = nrows >> 1;
                 for (int j = 0; j < nrows; ++j) {
                     const int4 r0 = __ldg((const int4*)(a.rows + row0 + j));
                     ccmin = fminf(ccmin, __int_as_float(r0.w));
@@ -233,7 +321,6 @@ conv_mc_tc_f32(const McTcArgs m) {
                     rmax = max(rmax, r0.y + r0.z - 1);
                     if (j == jc) {
                         const int4 r1 = __ldg((const int4*)(a.rows + row0 + j) + 1);
-                        yc0 = (uint32_t)r0.x;
                         cc0 = __int_as_float(r0.w);
                         const float sc0 = __int_as_float(r1.x), ik = a.isk;
                         p1 = -sc0 * ik;
@@ -241,17 +328,11 @@ conv_mc_tc_f32(const McTcArgs m) {
                         p3 = sc0 * ik * ik * ik * (1.0f / 6.0f);
                     }
                 }
-                xc0 = (uint32_t)(unsigned long long)__double2ll_rn((a.u0 + (double)(ix0 + ic) * a.du) * a.sx);
                 const float pad = 1e-3f * sqrtf(a.hmax);             // slack for the fp32 rounding of the extents
-#pragma unroll
-                for (int b = 0; b < 2; ++b) {
-                    // columns 8 b .. min(8 b + 7, ncols - 1), rows 4 b .. min(4 b + 3, nrows - 1); an empty quarter reaches nothing
-                    const int c0 = 8 * b, c1 = min(8 * b + 7, ncols - 1), r0 = 4 * b, r1 = min(4 * b + 3, nrows - 1);
-                    const float xa = (float)(c0 - ic) * a.duk, xb = (float)(c1 - ic) * a.duk;
-                    const float ya = (float)(r0 - jc) * a.dyk, yb = (float)(r1 - jc) * a.dyk;
-                    bxlo[b] = c1 >= c0 ? fminf(xa, xb) - pad : 1e30f; bxhi[b] = c1 >= c0 ? fmaxf(xa, xb) + pad : -1e30f;
-                    bylo[b] = r1 >= r0 ? fminf(ya, yb) - pad : 1e30f; byhi[b] = r1 >= r0 ? fmaxf(ya, yb) + pad : -1e30f;
-                }
+                const float xa = (float)(-ic) * a.duk, xb = (float)(ncols - 1 - ic) * a.duk;
+                const float ya = (float)(-jc) * a.dyk, yb = (float)(nrows - 1 - jc) * a.dyk;
+                xlo = fminf(xa, xb) - pad; xhi = fmaxf(xa, xb) + pad;
+                ylo = fminf(ya, yb) - pad; yhi = fmaxf(ya, yb) + pad;
                 ccmin *= 0.999f;
             }
             const float fxw = (float)(a.du >= 0.0 ? ix0 : ix0 + ncols - 1);
@@ -260,22 +341,28 @@ conv_mc_tc_f32(const McTcArgs m) {
             const Rec32* __restrict__ rec = a.rec;
             unsigned long long* tab_base = (unsigned long long*)(s_tc + kOffTabBase);
             int* tab_end = (int*)(s_tc + kOffTabEnd);
-            uint4* fifo_c = (uint4*)(s_tc + kOffFifoC);
+            float* fifo_x = (float*)(s_tc + kOffFifoX);
+            float* fifo_y = (float*)(s_tc + kOffFifoY);
+            float* fifo_c = (float*)(s_tc + kOffFifoC);
             uint32_t* fifo_i = (uint32_t*)(s_tc + kOffFifoI);
-            unsigned char* fifo_m = s_tc + kOffFifoM;
             volatile uint32_t* grp_n = (volatile uint32_t*)(s_tc + kOffGrpN);
             const float hlim = a.hmax * 1.0001f;
-
-            auto fetch = [&](int i, int total) -> uint4 {            // record number i of this pass's stream
+            // entry p of the FIFO: pair p >> 1, member p & 1; high part = multiple of 4096 units, low part = the rest
+            auto put = [&](int pos, int dxi, int dyi, float cs, float q, uint32_t sidx) {
+                const int p = pos & (kTcFifo - 1), o = 4 * (p >> 1) + (p & 1);
+                fifo_x[o] = (float)(dxi & ~0xfff); fifo_x[o + 2] = (float)(dxi & 0xfff);
+                fifo_y[o] = (float)(dyi & ~0xfff); fifo_y[o + 2] = (float)(dyi & 0xfff);
+                fifo_c[o] = cs; fifo_c[o + 2] = q;
+                fifo_i[p] = sidx;
+            };
+            // record number i of this pass's stream; `cur` is this lane's ring cursor (i only grows within a pass)
+            auto fetch = [&](int i, int total, int& cur) -> uint4 {
                 if (i >= total) return make_uint4(0, 0, 0, 0);
-                int lo = 0, hi = kTcRings - 1;                        // first ring whose end is beyond i
-                while (lo < hi) {
-                    const int mid = (lo + hi) >> 1;
-                    if (tab_end[mid] > i) hi = mid; else lo = mid + 1;
-                }
-                return ldg_rec(tab_base[lo], i);
+                while (tab_end[cur] <= i) ++cur;
+                return ldg_rec(tab_base[cur], i);
             };
 
+            PROF_DECL(4);
             int gpos = 0, published = 0;                              // candidates kept so far (FIFO position, unwrapped); groups published
             for (int pass = 0; rmin + pass * kTcRings <= rmax; ++pass) {
                 // ---- ring table of this pass: lane l of sub-pass t <-> ring number 32 t + l
@@ -321,277 +408,311 @@ conv_mc_tc_f32(const McTcArgs m) {
                 }
                 __syncwarp();
                 const int total = run;
-                // ---- the stream of this pass in blocks of 32, the next block's records in flight
-                uint4 nxt = fetch(lane, total);
+                // ---- the stream of this pass in blocks of 32, the records of the next three blocks in flight
+                int cur = 0;
+                uint4 n0 = fetch(lane, total, cur), n1 = fetch(32 + lane, total, cur), n2 = fetch(64 + lane, total, cur);
                 for (int base = 0; base < total; base += 32) {
-                    const uint4 raw = nxt;
-                    nxt = fetch(base + 32 + lane, total);
-                    unsigned reach = 0;
+                    const uint4 raw = n0;
+                    n0 = n1; n1 = n2;
+                    n2 = fetch(base + 96 + lane, total, cur);
+                    bool keep = false;
                     float cs = 0.f;
+                    const int dxi = (int)(raw.x - xc0), dyi = (int)(raw.y - yc0);
                     if (base + lane < total) {
-                        const float X = (float)(int)(raw.x - xc0) * sxk;
-                        const float Y = (float)(int)(raw.y - yc0) * syk;
+                        const float X = (float)dxi * sxk, Y = (float)dyi * syk;
                         cs = fmaf(Y, fmaf(Y, fmaf(Y, p3, p2), p1), cc0);
-                        const float cmin = ccmin * cs;
-                        float vx[2], uy[2];
-#pragma unroll
-                        for (int b = 0; b < 2; ++b) {
-                            const float ex = fmaxf(fmaxf(bxlo[b] - X, X - bxhi[b]), 0.0f), ey = fmaxf(fmaxf(bylo[b] - Y, Y - byhi[b]), 0.0f);
-                            vx[b] = ex * ex; uy[b] = ey * ey;
-                            if (MODE >= 1) { vx[b] = vx[b] * fmaf(vx[b], -a12, 1.0f); uy[b] = uy[b] * fmaf(uy[b], -a12, 1.0f); }
-                        }
-#pragma unroll
-                        for (int qq = 0; qq < 4; ++qq) reach |= fmaf(cmin, vx[qq & 1], uy[qq >> 1]) <= hlim ? 1u << qq : 0u;
+                        const float ex = fmaxf(fmaxf(xlo - X, X - xhi), 0.0f), ey = fmaxf(fmaxf(ylo - Y, Y - yhi), 0.0f);
+                        float v = ex * ex, u = ey * ey;
+                        if (MODE >= 1) { v = v * fmaf(v, -a12, 1.0f); u = u * fmaf(u, -a12, 1.0f); }
+                        keep = fmaf(ccmin * cs, v, u) <= hlim;
                     }
-                    const unsigned mk = __ballot_sync(0xffffffffu, reach != 0);
+                    const unsigned mk = __ballot_sync(0xffffffffu, keep);
                     const int nk = __popc(mk);
                     if (nk == 0) continue;
-                    // groups this block writes into for the first time must have been released by the compute warps
-                    const int g_first = (gpos + 15) >> 4, g_last = (gpos + nk - 1) >> 4;
+                    PROF_LAP(0);
+                    // groups this block writes into for the first time must have been released by their readers
+                    const int g_first = (gpos + kTcSC - 1) / kTcSC, g_last = (gpos + nk - 1) / kTcSC;
                     for (int gi = g_first; gi <= g_last; ++gi)
                         if (gi >= kTcGroups) mbar_wait(b_cempty + 8 * (gi % kTcGroups), (uint32_t)(gi / kTcGroups - 1) & 1u);
-                    if (reach != 0) {
-                        const int p = (gpos + __popc(mk & ((1u << lane) - 1u))) & (kTcFifo - 1);
-                        fifo_c[p] = make_uint4(raw.x, raw.y, __float_as_uint(cs), raw.w);
-                        fifo_i[p] = raw.z;
-                        fifo_m[p] = (unsigned char)reach;
-                    }
+                    PROF_LAP(1);
+                    if (keep) put(gpos + __popc(mk & ((1u << lane) - 1u)), dxi, dyi, cs, __uint_as_float(raw.w), raw.z);
                     __syncwarp();
                     gpos += nk;
                     // publish the complete groups that are known not to be the last one (a later candidate exists)
-                    const int p_end = (gpos - 1) >> 4;
+                    const int p_end = (gpos - 1) / kTcSC;
                     if (lane == 0)
                         for (int gi = published; gi < p_end; ++gi) {
-                            grp_n[gi % kTcGroups] = 16u;
+                            grp_n[gi % kTcGroups] = (uint32_t)kTcSC;
                             mbar_arrive(b_cfull + 8 * (gi % kTcGroups));
                         }
                     published = max(published, p_end);
                 }
             }
-            // ---- the last group (1 .. 16 candidates; none at all: an empty group 0) carries the end-of-tile mark
-            __syncwarp();
-            if (lane == 0) {
-                const int gi = gpos > 0 ? (gpos - 1) >> 4 : 0;
-                grp_n[gi % kTcGroups] = (uint32_t)(gpos - 16 * gi) | 0x80u;
-                mbar_arrive(b_cfull + 8 * (gi % kTcGroups));
+#ifdef HCG_TC_PROF
+            if (PROF_ON) printf("STREAM: kept %d total %lld | work %lld wait_cempty %lld\n", gpos, clock64() - prof_t0_, prof_[0], prof_[1]);
+#endif
+            // ---- the last group (1 .. kTcSC candidates; none at all: an empty group 0) carries the end-of-tile mark;
+            // its unused slots are filled with candidates far outside every cell's reach (weight 0, never counted)
+            {
+                const int gi = gpos > 0 ? (gpos - 1) / kTcSC : 0;
+                const int nlast = gpos - kTcSC * gi;
+                const int far = __float2int_rn((8.0f * fabsf(a.dyk) + 10.0f * sqrtf(a.hmax)) / syk);
+                if (gpos > 0 && lane >= nlast) put(kTcSC * gi + lane, 0, far, 1.0f, 0.0f, 0u);
+                __syncwarp();
+                if (lane == 0) {
+                    grp_n[gi % kTcGroups] = (uint32_t)nlast | 0x80u;
+                    mbar_arrive(b_cfull + 8 * (gi % kTcGroups));
+                }
             }
-        } else {
-            // ============================================================ spectrum rows (B): 64 threads, one 16-byte unit per row each
-            const int t2 = (warp - kTcCW - 2) * 32 + lane;           // 0 .. 63
-            const int upr = nch >> 2;                                 // 16-byte units per row (<= 64)
-            const bool on = t2 < upr;
-            uint32_t off_u[4];                                        // offset of unit t2 in a K-step's B region, by row & 3
+        }
+    } else if (warp >= kTcCW) {
+        // ================================================================ spectrum rows (B): 128 threads
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+        // thread t4: 16-byte unit u = t4 & 63 of the rows r = 2 i + (t4 >> 6), i = 0 .. kTcSC / 2 - 1, of every stage
+        const int t4 = tid - kTcCT;
+        const int u = t4 & 63, rp = t4 >> 6;
+        const int upr = nch >> 2;                                     // 16-byte units per row (<= 64)
+        const bool on = u < upr;
+        // offset of unit u in a K-step's B region for a row r: by r & 3 (row in the 4-row atom), plus ((r >> 2) & 1) * 512, (r >> 3) * 8192
+        uint32_t off_u[2];
 #pragma unroll
-            for (int k3 = 0; k3 < 4; ++k3)
-                off_u[k3] = (uint32_t)((t2 >> 3) * 1024 + k3 * 128 + (((((t2 & 7) >> 1) ^ k3) << 5) | ((t2 & 1) << 4)));
-            const unsigned long long vsrc = (unsigned long long)(uintptr_t)(m.values + ch0 + 4 * (on ? t2 : 0));
-            const uint32_t vstride = (uint32_t)m.nchan * 4u;          // bytes per row
-            const uint32_t fifo_i_s = s_base + kOffFifoI, grp_n_s = s_base + kOffGrpN;
-            int nst = 0x7fffffff, pf = 0;
-            for (int k = 0;; ++k) {
-                // request the rows of the stages up to k + P (zeros for the missing rows of the last stage)
-                while (pf <= k + kTcP) {
+        for (int h = 0; h < 2; ++h) {
+            const int k3 = 2 * h + rp;                                // r & 3 for r = 2 i + rp: i even -> rp, i odd -> 2 + rp
+            off_u[h] = (uint32_t)((u >> 3) * 1024 + k3 * 128 + (((((u & 7) >> 1) ^ k3) << 5) | ((u & 1) << 4)));
+        }
+        const unsigned long long vsrc = (unsigned long long)(uintptr_t)(m.values + ch0 + 4 * (on ? u : 0));
+        const uint32_t vstride = (uint32_t)m.nchan * 4u;              // bytes per row
+        const uint32_t fifo_i_s = s_base + kOffFifoI, grp_n_s = s_base + kOffGrpN;
+        // row r = 2 i + rp of the stage: (r >> 3) = i >> 2, (r >> 2) & 1 = (i >> 1) & 1, r & 3 = 2 (i & 1) + rp
+        auto unit_off = [&](int i) -> uint32_t { return (uint32_t)((i >> 2) * 8192 + ((i >> 1) & 1) * 512) + off_u[i & 1]; };
+        constexpr int NU = kTcSC / 2;                                 // units per thread per stage
+        PROF_DECL(8);
+        int nst = 0x7fffffff, pf = 0;
+        for (int k = 0;; ++k) {
+            // request the rows of the stages up to k + BD (the missing rows of the last stage are zeros)
+            while (pf <= k + kTcBD) {
+                if (pf < nst) {
+                    const int grp = pf % kTcGroups, slot = pf % kTcNS;
+                    PROF_LAP(0);
+                    mbar_wait(b_cfull + 8 * grp, (uint32_t)(pf / kTcGroups) & 1u);
+                    PROF_LAP(1);
+                    const uint32_t info = lds_u1(grp_n_s + 4u * (uint32_t)grp);
+                    const int n = (int)(info & 0x7fu);
+                    if (info & 0x80u) nst = n > 0 ? pf + 1 : pf;
                     if (pf < nst) {
-                        const int grp = pf % kTcGroups, slot = pf % kTcNS;
-                        mbar_wait(b_cfull + 8 * grp, (uint32_t)(pf / kTcGroups) & 1u);
-                        const uint32_t info = lds_u1(grp_n_s + 4u * (uint32_t)grp);
-                        const int n = (int)(info & 31u);
-                        if (info & 0x80u) nst = n > 0 ? pf + 1 : pf;
-                        if (pf < nst) {
-                            if (pf >= kTcNS) mbar_wait(b_empty + 8 * slot, (uint32_t)(pf / kTcNS - 1) & 1u);
-                            const uint32_t sb = s_base + (uint32_t)slot * kStageBytes + kOffBraw;
-                            if (on) {
-                                uint32_t idx[16];
+                        if (pf >= kTcNS) mbar_wait(b_empty + 8 * slot, (uint32_t)(pf / kTcNS - 1) & 1u);
+                        PROF_LAP(2);
+                        const uint32_t sb = s_base + (uint32_t)slot * kStageBytes + kOffBraw;
+#ifdef HCG_TC_NOB
+                        if (false) {
+#else
+                        if (on) {
+#endif
 #pragma unroll
-                                for (int r = 0; r < 16; ++r) idx[r] = lds_u1(fifo_i_s + (uint32_t)grp * 64u + 4u * r);
+                            for (int i0 = 0; i0 < NU; i0 += 8) {
+                                uint32_t idx[8];
 #pragma unroll
-                                for (int r = 0; r < 16; ++r) {
-                                    const uint32_t dst = sb + (uint32_t)((r >> 3) * 8192 + ((r >> 2) & 1) * 512) + off_u[r & 3];
-                                    if (r < n) cp_async16_cg(dst, (const void*)(uintptr_t)(vsrc + (unsigned long long)idx[r] * vstride));
+                                for (int i = 0; i < 8; ++i) idx[i] = lds_u1(fifo_i_s + (uint32_t)(grp * kTcSC + 2 * (i0 + i) + rp) * 4u);
+#pragma unroll
+                                for (int i = 0; i < 8; ++i) {
+                                    const uint32_t dst = sb + unit_off(i0 + i);
+                                    if (2 * (i0 + i) + rp < n) cp_async16_cg(dst, (const void*)(uintptr_t)(vsrc + (unsigned long long)idx[i] * vstride));
                                     else sts_u4(dst, make_uint4(0, 0, 0, 0));
                                 }
                             }
-                            __syncwarp();
-                            if (lane == 0) mbar_arrive(b_cempty + 8 * grp);   // done with the group's sample indices
                         }
-                    }
-                    cp_commit();
-                    ++pf;
-                }
-                if (k >= nst) {
-                    if (nst == 0 && lane == 0) mbar_arrive(b_full);   // empty tile: the compute warps release the MMA warp through stage 0
-                    break;
-                }
-                // the rows of stage k have landed (each thread reads back its own bytes): lo = v - trunc_tf32(v)
-                cp_wait<kTcP>();
-                const int slot = k % kTcNS;
-                const uint32_t sb = s_base + (uint32_t)slot * kStageBytes + kOffBraw;
-                if (on) {
-#pragma unroll
-                    for (int r0 = 0; r0 < 16; r0 += 4) {
-                        uint4 v[4];
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) {
-                            const int r = r0 + j;
-                            v[j] = lds_u4(sb + (uint32_t)((r >> 3) * 8192 + ((r >> 2) & 1) * 512) + off_u[r & 3]);
-                        }
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) {
-                            const int r = r0 + j;
-                            uint4 l;
-                            l.x = __float_as_uint(__uint_as_float(v[j].x) - __uint_as_float(v[j].x & 0xffffe000u));
-                            l.y = __float_as_uint(__uint_as_float(v[j].y) - __uint_as_float(v[j].y & 0xffffe000u));
-                            l.z = __float_as_uint(__uint_as_float(v[j].z) - __uint_as_float(v[j].z & 0xffffe000u));
-                            l.w = __float_as_uint(__uint_as_float(v[j].w) - __uint_as_float(v[j].w & 0xffffe000u));
-                            sts_u4(sb + (uint32_t)(kOffBlo - kOffBraw + (r >> 3) * 8192 + ((r >> 2) & 1) * 512) + off_u[r & 3], l);
-                        }
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(b_cempty + 8 * grp);   // done with the group's sample indices
                     }
                 }
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                __syncwarp();
-                if (lane == 0) mbar_arrive(b_full + 8 * slot);
+                cp_commit();
+                ++pf;
             }
-            cp_wait<0>();
+            if (k >= nst) break;
+            // the rows of stage k have landed (each thread reads back its own bytes): lo = v - trunc_tf32(v)
+            PROF_LAP(0);
+            cp_wait<kTcBD>();
+            PROF_LAP(3);
+            const int slot = k % kTcNS;
+            const uint32_t sb = s_base + (uint32_t)slot * kStageBytes + kOffBraw;
+#ifdef HCG_TC_NOB
+            if (false) {
+#else
+            if (on) {
+#endif
+#pragma unroll
+                for (int i0 = 0; i0 < NU; i0 += 4) {
+                    uint4 v[4];
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) v[j] = lds_u4(sb + unit_off(i0 + j));
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        uint4 l;
+                        l.x = __float_as_uint(__uint_as_float(v[j].x) - __uint_as_float(v[j].x & 0xffffe000u));
+                        l.y = __float_as_uint(__uint_as_float(v[j].y) - __uint_as_float(v[j].y & 0xffffe000u));
+                        l.z = __float_as_uint(__uint_as_float(v[j].z) - __uint_as_float(v[j].z & 0xffffe000u));
+                        l.w = __float_as_uint(__uint_as_float(v[j].w) - __uint_as_float(v[j].w & 0xffffe000u));
+                        sts_u4(sb + (kOffBlo - kOffBraw) + unit_off(i0 + j), l);
+                    }
+                }
+            }
+            PROF_LAP(4);
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) mbar_arrive(b_bfull + 8 * slot);
+            PROF_LAP(5);
         }
+        cp_wait<0>();
+#ifdef HCG_TC_PROF
+        if (PROF_ON && warp == kTcCW) printf("BROWS: total %lld | issue %lld wait_cfull %lld wait_empty %lld cp_wait %lld split %lld fence+arrive %lld\n", clock64() - prof_t0_, prof_[0], prof_[1], prof_[2], prof_[3], prof_[4], prof_[5]);
+#endif
     } else {
-        // ================================================================ producers of A and B, accumulators
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 216;");
-        // MMA row (= TMEM lane) 32 q + l  <->  cell (8 (q & 1) + (l & 7), 4 (q >> 1) + (l >> 3)): a warp owns an
-        // 8 x 4-cell quarter of the tile; g selects the K-step of a stage (A) and the channel half (drain).
+        // ================================================================ A (kernel weights) and the accumulators
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 200;");
+        // MMA row (= TMEM lane) 32 q + l  <->  cell (8 (q & 1) + (l & 7), 4 (q >> 1) + (l >> 3)); g selects the half
+        // of a stage's K-steps (A) and the channel half (drain).
         const int q = warp & 3, g = warp >> 2;
         const int cell = q * 32 + lane;
         const int cix = 8 * (q & 1) + (lane & 7), ciy = 4 * (q >> 1) + (lane >> 3);
         const bool cell_ok = cix < ncols && ciy < nrows;
-        uint32_t xc, yc;
-        float cc;
+        // this cell's offset from the tile centre in fixed-point units, split like the candidates' (negated: the
+        // differences are formed by additions)
+        unsigned long long ncxh, ncxl, ncyh, ncyl, cc2;
         {
             const int4 r0 = __ldg((const int4*)(a.rows + min(row0 + ciy, a.ny - 1)));
-            yc = (uint32_t)r0.x;
-            cc = __int_as_float(r0.w);
-            xc = (uint32_t)(unsigned long long)__double2ll_rn((a.u0 + (double)(ix0 + min(cix, ncols - 1)) * a.du) * a.sx);
+            const uint32_t xc = (uint32_t)(unsigned long long)__double2ll_rn((a.u0 + (double)(ix0 + min(cix, ncols - 1)) * a.du) * a.sx);
+            const int cxi = (int)(xc - xc0), cyi = (int)((uint32_t)r0.x - yc0);
+            const float xh = -(float)(cxi & ~0xfff), xl = -(float)(cxi & 0xfff), yh = -(float)(cyi & ~0xfff), yl = -(float)(cyi & 0xfff);
+            const float cc = __int_as_float(r0.w);
+            ncxh = f2_pack(xh, xh); ncxl = f2_pack(xl, xl); ncyh = f2_pack(yh, yh); ncyl = f2_pack(yl, yl); cc2 = f2_pack(cc, cc);
         }
         float hm = cell_ok ? a.hmax : -1.0f;
-        const float sxk = a.sxk, syk = a.syk, a12 = a.a12;
-        HCG_PIN(xc); HCG_PIN(yc);
-        asm volatile("" : "+f"(cc), "+f"(hm));
-        const uint32_t fifo_c_s = s_base + kOffFifoC, fifo_m_s = s_base + kOffFifoM;
+        asm volatile("" : "+l"(ncxh), "+l"(ncxl), "+l"(ncyh), "+l"(ncyl), "+l"(cc2), "+f"(hm));
+        const unsigned long long sxk2 = f2_pack(a.sxk, a.sxk), syk2 = f2_pack(a.syk, a.syk);
+        const unsigned long long na12 = f2_pack(-a.a12, -a.a12), pa12 = f2_pack(a.a12, a.a12), one2 = f2_pack(1.0f, 1.0f);
+        const uint32_t fifo_x_s = s_base + kOffFifoX, fifo_y_s = s_base + kOffFifoY, fifo_c_s = s_base + kOffFifoC;
         const uint32_t grp_n_s = s_base + kOffGrpN;
-
-        // ---- A: this thread owns the 8 candidates of K-step g of a stage for its cell (rows of 8 weights: two 16-byte halves)
-        uint32_t a_off = (uint32_t)(g * 4096 + (cell >> 3) * 128 + (cell & 7) * 16);
-        HCG_PIN(a_off);
+        const uint32_t t_lane = tm + ((uint32_t)(q * 32) << 16);     // this warp's TMEM lanes
 
         float acc[128];
 #pragma unroll
         for (int j = 0; j < 128; ++j) acc[j] = 0.0f;
-        float wsum = 0.0f;
+        unsigned long long wsum2 = 0ull;
         int csum = 0;
 
+        // take a finished chunk over from the TMEM accumulator: channels 128 g .. 128 g + 127 of this thread's cell
         auto drain = [&](int j) {
-            const int buf = j & 1;
-            mbar_wait(b_dfull + 8 * buf, (uint32_t)(j >> 1) & 1u);
+            mbar_wait(b_dfull, (uint32_t)j & 1u);
             tc_fence_after();
-            const uint32_t ta = tm + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * 256 + g * 128);
 #pragma unroll
-            for (int h = 0; h < 4; ++h) {
-                uint32_t v[32];
-                tmem_ld32(ta + 32 * h, v);
+            for (int h = 0; h < 8; ++h) {
+                uint32_t v[16];
+                tmem_ld16(t_lane + (uint32_t)(g * 128 + 16 * h), v);
                 tmem_ld_wait();
 #pragma unroll
-                for (int c = 0; c < 32; ++c) acc[32 * h + c] += __uint_as_float(v[c]);
+                for (int c = 0; c < 16; ++c) acc[16 * h + c] += __uint_as_float(v[c]);
             }
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(b_dempty + 8 * buf);
-        };
-
-        // one candidate of the group against this thread's cell: q w(d) where d <= R, else 0
-        auto pair_weight = [&](const uint4 e) -> float {
-            const float dy = (float)(int)(e.y - yc) * syk;
-            const float dx = (float)(int)(e.x - xc) * sxk;
-            float u = dy * dy, v = dx * dx;
-            if (MODE >= 1) { u = u * fmaf(u, -a12, 1.0f); v = v * fmaf(v, -a12, 1.0f); }
-            const float h = fmaf(cc * __uint_as_float(e.z), v, u);
-            const float ee = MODE == 2 ? h * fmaf(h, a12, 1.0f) : h;
-            const float w = ex2_approx(-ee) * __uint_as_float(e.w);
-            const bool hit = h <= hm;
-            if (COUNTS) csum += hit ? 1 : 0;
-            return hit ? w : 0.0f;
-        };
-        auto store_weight = [&](uint32_t ad, int j, float ws) {     // slot j of the K-step: hi and lo parts
-            const float hi = __uint_as_float((__float_as_uint(ws) + 0x1000u) & 0xffffe000u);
-            const uint32_t p = ad + (uint32_t)((j >> 2) * 2048 + (j & 3) * 4);
-            asm volatile("st.shared.f32 [%0], %1;" ::"r"(p + kOffAhi), "f"(hi) : "memory");
-            asm volatile("st.shared.f32 [%0], %1;" ::"r"(p + kOffAlo), "f"(ws - hi) : "memory");
+            if (lane == 0) mbar_arrive(b_dempty);
         };
 
         int k = 0, jd = 0, nst = 0x7fffffff;
+        PROF_DECL(8);
         for (;;) {
             if (k >= nst) break;                                     // the last group has been seen
+            // the chunk the MMA warp has finished must be taken over before it can start the next: as soon as it is
+            // complete, and at the latest when this warp would have to wait for a stage of the following chunk
+            if (jd < k / kTcCH && (k == (jd + 1) * kTcCH + kTcNS - 1 || mbar_test(b_dfull, (uint32_t)jd & 1u))) {
+                PROF_LAP(0); drain(jd); ++jd; PROF_LAP(5);
+            }
+            PROF_LAP(0);
             mbar_wait(b_cfull + 8 * (k % kTcGroups), (uint32_t)(k / kTcGroups) & 1u);
+            PROF_LAP(1);
             const uint32_t info = lds_u1(grp_n_s + 4u * (uint32_t)(k % kTcGroups));
-            const int ng = (int)(info & 31u);
-            if (info & 0x80u) nst = ng > 0 ? k + 1 : k;
+            if (info & 0x80u) nst = (info & 0x7fu) > 0 ? k + 1 : k;
             if (k >= nst) break;
             const int slot = k % kTcNS;
-            if (k >= kTcNS) mbar_wait(b_empty + 8 * slot, (uint32_t)(k / kTcNS - 1) & 1u);
-            const uint32_t ad = s_base + (uint32_t)slot * kStageBytes + a_off;
-
-            // ---- A: the candidates of K-step g that can reach this warp's quarter, two at a time; zeros elsewhere
-            {
-                const uint32_t e0 = (uint32_t)(k % kTcGroups) * 16u + (uint32_t)g * 8u;   // FIFO index of the first
-                const uint2 mk = lds_u2(fifo_m_s + e0);
-                sts_u4(ad + kOffAhi, make_uint4(0, 0, 0, 0));
-                sts_u4(ad + kOffAhi + 2048, make_uint4(0, 0, 0, 0));
-                sts_u4(ad + kOffAlo, make_uint4(0, 0, 0, 0));
-                sts_u4(ad + kOffAlo + 2048, make_uint4(0, 0, 0, 0));
-                // bit j: candidate j of the K-step reaches quarter q (reach masks are bytes: bit q of byte j)
-                const uint32_t sel = 0x01010101u << q;
-                uint32_t live = 0;
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    live |= ((mk.x & sel) >> (8 * j + q) & 1u) << j;
-                    live |= ((mk.y & sel) >> (8 * j + q) & 1u) << (4 + j);
-                }
-                const int nk = ng - g * 8;                            // candidates present in this K-step (may be <= 0 or >= 8)
-                live &= nk >= 8 ? 0xffu : (nk <= 0 ? 0u : (1u << nk) - 1u);
-                while (live) {                                        // warp-uniform
-                    const int j0 = __ffs(live) - 1;
-                    live &= live - 1;
-                    const bool two = live != 0;
-                    const int j1 = two ? __ffs(live) - 1 : j0;
-                    live &= live - 1;
-                    const uint4 ea = lds_u4(fifo_c_s + (e0 + j0) * 16u), eb = lds_u4(fifo_c_s + (e0 + j1) * 16u);
-                    const float wa = pair_weight(ea);
-                    const float wb = two ? pair_weight(eb) : 0.0f;
-                    wsum += wa;
-                    wsum += wb;
-                    store_weight(ad, j0, wa);
-                    if (two) store_weight(ad, j1, wb);
-                }
+            if (k >= kTcNS) {
+                mbar_wait(b_empty + 8 * slot, (uint32_t)(k / kTcNS - 1) & 1u);
+                tc_fence_after();
             }
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            PROF_LAP(2);
+
+            // ---- A: K-steps g * kTcKS / 2 .. of the stage x this thread's cell, two candidates per instruction
+#pragma unroll
+            for (int kk = 0; kk < kTcKS / 2; ++kk) {
+                const int ks = g * (kTcKS / 2) + kk;
+                const uint32_t pr0 = (uint32_t)((k % kTcGroups) * (kTcSC / 2) + ks * 4);   // first candidate pair of the K-step
+                uint32_t hi[8], lo[8];
+#pragma unroll
+                for (int pp = 0; pp < 4; ++pp) {
+                    const uint4 ex = lds_u4(fifo_x_s + (pr0 + pp) * 16u), ey = lds_u4(fifo_y_s + (pr0 + pp) * 16u);
+                    const uint4 ec = lds_u4(fifo_c_s + (pr0 + pp) * 16u);
+                    const unsigned long long xh = ((unsigned long long)ex.y << 32) | ex.x, xl = ((unsigned long long)ex.w << 32) | ex.z;
+                    const unsigned long long yh = ((unsigned long long)ey.y << 32) | ey.x, yl = ((unsigned long long)ey.w << 32) | ey.z;
+                    const unsigned long long cs = ((unsigned long long)ec.y << 32) | ec.x, qq = ((unsigned long long)ec.w << 32) | ec.z;
+                    // exact differences of the split fixed-point offsets, one rounding in the last addition
+                    const unsigned long long dx = f2_mul(f2_add(f2_add(xh, ncxh), f2_add(xl, ncxl)), sxk2);
+                    const unsigned long long dy = f2_mul(f2_add(f2_add(yh, ncyh), f2_add(yl, ncyl)), syk2);
+                    unsigned long long v = f2_mul(dx, dx), u = f2_mul(dy, dy);
+                    if (MODE >= 1) { v = f2_mul(v, f2_fma(v, na12, one2)); u = f2_mul(u, f2_fma(u, na12, one2)); }
+                    const unsigned long long h2 = f2_fma(f2_mul(cc2, cs), v, u);
+                    const unsigned long long e2 = MODE == 2 ? f2_mul(h2, f2_fma(h2, pa12, one2)) : h2;
+                    float ha, hb, ea, eb;
+                    f2_unpack(h2, ha, hb);
+                    f2_unpack(e2, ea, eb);
+                    const unsigned long long w2 = f2_mul(f2_pack(ex2_approx(-ea), ex2_approx(-eb)), qq);
+                    float wa, wb;
+                    f2_unpack(w2, wa, wb);
+                    const bool hita = ha <= hm, hitb = hb <= hm;
+                    wa = hita ? wa : 0.0f;
+                    wb = hitb ? wb : 0.0f;
+                    if (COUNTS) csum += (hita ? 1 : 0) + (hitb ? 1 : 0);
+                    const unsigned long long ws2 = f2_pack(wa, wb);
+                    wsum2 = f2_add(wsum2, ws2);
+                    hi[2 * pp] = (__float_as_uint(wa) + 0x1000u) & 0xffffe000u;
+                    hi[2 * pp + 1] = (__float_as_uint(wb) + 0x1000u) & 0xffffe000u;
+                    lo[2 * pp] = __float_as_uint(wa - __uint_as_float(hi[2 * pp]));
+                    lo[2 * pp + 1] = __float_as_uint(wb - __uint_as_float(hi[2 * pp + 1]));
+                }
+                const uint32_t t_hi = t_lane + kTmemA + (uint32_t)(slot * kTmemAStage + ks * 8), t_lo = t_hi + 8 * kTcKS;
+                asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
+                             ::"r"(t_hi), "r"(hi[0]), "r"(hi[1]), "r"(hi[2]), "r"(hi[3]), "r"(hi[4]), "r"(hi[5]), "r"(hi[6]), "r"(hi[7]) : "memory");
+                asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
+                             ::"r"(t_lo), "r"(lo[0]), "r"(lo[1]), "r"(lo[2]), "r"(lo[3]), "r"(lo[4]), "r"(lo[5]), "r"(lo[6]), "r"(lo[7]) : "memory");
+            }
+            PROF_LAP(3);
+            tmem_st_wait();
+            PROF_LAP(4);
+            tc_fence_before();
             if (tid == 0) s_flag[slot] = k == nst - 1 ? 1u : 0u;
             __syncwarp();
             if (lane == 0) {
                 mbar_arrive(b_cempty + 8 * (k % kTcGroups));          // this warp is done with the group's FIFO entries
-                mbar_arrive(b_full + 8 * slot);
+                mbar_arrive(b_afull + 8 * slot);
             }
-            if (k >= (jd + 1) * kTcCH + kTcNS) { drain(jd); ++jd; }
+            PROF_LAP(6);
             ++k;
         }
+#ifdef HCG_TC_PROF
+        if (PROF_ON && warp == 0) printf("COMPUTE: stages %d total %lld | misc %lld wait_cfull %lld wait_empty %lld agen %lld wait_st %lld fence+arrive %lld drain %lld\n",
+                                        k, clock64() - prof_t0_, prof_[0], prof_[1], prof_[2], prof_[3], prof_[4], prof_[6], prof_[5]);
+#endif
         if (nst == 0) {                                              // nothing can reach this tile: release the MMA warp
             if (tid == 0) s_flag[0] = 3u;
             __syncwarp();
-            if (lane == 0) mbar_arrive(b_full);
+            if (lane == 0) mbar_arrive(b_afull);
         }
         for (const int nchunk = (nst + kTcCH - 1) / kTcCH; jd < nchunk; ++jd) drain(jd);
 
         // ---- finish: W and counts over the two K-step halves of a cell (fixed order), normalise, store
+        float wsa, wsb;
+        f2_unpack(wsum2, wsa, wsb);
         bar_compute();                                               // every warp is done with the FIFO: reuse it
-        float* s_w = (float*)(s_tc + kOffFifoC);
+        float* s_w = (float*)(s_tc + kOffFifoX);
         int* s_c = (int*)(s_w + 2 * 128);
-        s_w[g * 128 + cell] = wsum;
+        s_w[g * 128 + cell] = wsa + wsb;
         if (COUNTS) s_c[g * 128 + cell] = csum;
         // 0 * inf = NaN reaches every cell of the tile: non-finite sums flag the tile for the cell-by-cell pass
         float chk = 0.0f;
@@ -626,7 +747,7 @@ conv_mc_tc_f32(const McTcArgs m) {
 
     tc_fence_before();
     __syncthreads();
-    if (warp == kTcCW) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tm), "r"(512u));
+    if (warp == kMmaWarp) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tm), "r"(512u));
 }
 
 int launch_conv_mc_tc(hcgrid_ctx* c, const float* values, int nchan, float* cube, float* wmap, int32_t* counts,
