@@ -308,7 +308,7 @@ def run_product(args):
             if args.scale == 1.0 and (args.config, st["kernel"]) in NCU_TRAFFIC else None),
         "traffic_source": NCU_TRAFFIC.get((args.config, st["kernel"]), (None, None))[1] if args.traffic is None else "--traffic",
         "kernel": {1: "conv1_simple_f32", 2: "conv1_staged_f32", 3: "conv_general<f32>", 4: "conv_general<f64 pair>",
-                   5: "conv_general<f64>", 6: "conv1_tile_f32", 7: "conv_mc_f32"}.get(st["kernel"], str(st["kernel"])),
+                   5: "conv_general<f64>", 6: "conv1_tile_f32", 7: "conv_mc_f32", 8: "conv_mc_tc_f32"}.get(st["kernel"], str(st["kernel"])),
         "kernel_us": t_conv * 1e6, "t_roof_us": mdl["t_roof_s"] * 1e6,
         "legs_us": {"fp32": mdl["t_fp32_s"] * 1e6, "mufu": mdl["t_mufu_s"] * 1e6, "hbm": mdl["t_hbm_s"] * 1e6},
         "n_hit": n_hit, "n_cand": cand["n_cand"], "n_cand_rows_counted": cand["rows_counted"],

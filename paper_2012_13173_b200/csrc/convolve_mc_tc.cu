@@ -48,7 +48,8 @@ constexpr int kTcTX = 16, kTcTY = 8;           // tile = 128 cells = MMA M
 constexpr int kTcCW = 8;                       // compute warps (warps 0 .. 7)
 constexpr int kTcCT = kTcCW * 32;              // compute threads
 constexpr int kTcBW = 4;                       // spectrum-row warps (warps 8 .. 11)
-constexpr int kTcThreads = kTcCT + 32 * kTcBW + 128;   // + the service warpgroup: MMA issuer, stream builder, two idle warps
+constexpr int kTcSW = 3;                       // stream-builder warps
+constexpr int kTcThreads = kTcCT + 32 * kTcBW + 128;   // + the service warpgroup: MMA issuer, three stream builders
 constexpr int kTcKS = 4;                       // K-steps (of 8 candidates) per pipeline stage
 constexpr int kTcSC = 8 * kTcKS;               // candidates per stage = per FIFO group
 constexpr int kTcNS = 3;                       // pipeline stages (B in shared memory, A in tensor memory)
@@ -72,7 +73,7 @@ constexpr int kOffTabEnd = kOffTabBase + kTcRings * 8;     // int [kTcRings]
 constexpr int kOffGrpN = kOffTabEnd + kTcRings * 4;        // uint32 [kTcGroups]: candidates in the group | 0x80 (last group of the tile)
 constexpr int kOffBars = kOffGrpN + kTcGroups * 4;         // u64: afull[NS], bfull[NS], empty[NS], dfull, dempty, cfull[G], cempty[G]
 constexpr int kOffMisc = kOffBars + 8 * (3 * kTcNS + 2 + 2 * kTcGroups);
-constexpr int kTcSmem = kOffMisc + 64;
+constexpr int kTcSmem = kOffMisc + 64 + 8 + 4 * kTcGroups;   // flags, tmem address, token, group counters
 static_assert(kTcSmem <= 227 * 1024, "shared memory");
 
 // ---- PTX wrappers
@@ -83,14 +84,14 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 // Bounded: a wait that outlasts any legitimate one (seconds) is a broken pipeline -- fail loudly, do not hang.
-// The suspend-time hint keeps a waiting warp off the issue slots of the working ones (it still wakes when the phase completes).
+// (No suspend-time hint: with one, a wait on an already completed phase took ~700 cycles instead of ~100.)
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     for (uint32_t spins = 0;; ++spins) {
         uint32_t ok;
-        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                     : "=r"(ok) : "r"(bar), "r"(parity), "r"(20000u) : "memory");
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
         if (ok) return;
-        if (spins > (1u << 20)) __trap();
+        if (spins > (1u << 24)) __trap();
     }
 }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -225,6 +226,8 @@ conv_mc_tc_f32(const McTcArgs m) {
     volatile uint32_t* s_flag = (volatile uint32_t*)(s_tc + kOffMisc);   // [NS] stage flags
     uint32_t* s_tmem = (uint32_t*)(s_tc + kOffMisc + 4 * kTcNS);
     int* s_bad = (int*)(s_tmem + 1);
+    volatile int* s_tok = (volatile int*)(s_tc + kOffMisc + 64);    // [0] next stream block to append, [1] FIFO position
+    int* s_gcnt = (int*)(s_tc + kOffMisc + 72);                     // [G] candidates written into each FIFO group
 
     const int tile = blockIdx.x;
     const int ch0 = blockIdx.y * 256;
@@ -251,6 +254,8 @@ conv_mc_tc_f32(const McTcArgs m) {
             mbar_init(b_dfull, 1); mbar_init(b_dempty, kTcCW);
             for (int j = 0; j < kTcGroups; ++j) { mbar_init(b_cfull + 8 * j, 1); mbar_init(b_cempty + 8 * j, kTcCW + kTcBW); }
             *s_bad = 0;
+            s_tok[0] = 0; s_tok[1] = 0;
+            for (int j = 0; j < kTcGroups; ++j) s_gcnt[j] = 0;
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
     }
@@ -299,6 +304,9 @@ conv_mc_tc_f32(const McTcArgs m) {
                         if (s % kTcCH == kTcCH - 1 || (flag & 1u)) tc_commit(b_dfull);
                     }
                     __syncwarp();
+                } else if (s % kTcCH != 0) {                          // end-of-tile mark without a stage: close the open chunk
+                    if (lane == 0) tc_commit(b_dfull);
+                    __syncwarp();
                 }
                 if (flag & 1u) {
 #ifdef HCG_TC_PROF
@@ -307,8 +315,11 @@ conv_mc_tc_f32(const McTcArgs m) {
                     break;
                 }
             }
-        } else if (warp == kStreamWarp) {
-            // ============================================================ stream builder: steps (i)-(iii) + compaction
+        } else {
+            // ============================================================ stream builders: steps (i)-(iii) + compaction
+            // Three warps share the stream: warp sw tests blocks sw, sw + 3, ... of 32 records; a token handed on in
+            // block order gives every block its place in the FIFO, so the kept candidates stay in stream order.
+            const int sw = warp - kStreamWarp;
             float cc0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f, ccmin = 2.0f;
             float xlo, xhi, ylo, yhi;                                // extent of the tile's cell centres (scaled units)
             int rmin = 0x7fffffff, rmax = -0x7fffffff;
@@ -340,13 +351,14 @@ conv_mc_tc_f32(const McTcArgs m) {
             const bool flip = (ty & 1) != 0;                          // odd tile rows walk the rings south to north
             const Rec32* __restrict__ rec = a.rec;
             unsigned long long* tab_base = (unsigned long long*)(s_tc + kOffTabBase);
-            int* tab_end = (int*)(s_tc + kOffTabEnd);
+            volatile int* tab_end = (volatile int*)(s_tc + kOffTabEnd);
             float* fifo_x = (float*)(s_tc + kOffFifoX);
             float* fifo_y = (float*)(s_tc + kOffFifoY);
             float* fifo_c = (float*)(s_tc + kOffFifoC);
             uint32_t* fifo_i = (uint32_t*)(s_tc + kOffFifoI);
             volatile uint32_t* grp_n = (volatile uint32_t*)(s_tc + kOffGrpN);
             const float hlim = a.hmax * 1.0001f;
+            auto bar_stream = [&]() { asm volatile("bar.sync 2, %0;" ::"n"(32 * kTcSW) : "memory"); };
             // entry p of the FIFO: pair p >> 1, member p & 1; high part = multiple of 4096 units, low part = the rest
             auto put = [&](int pos, int dxi, int dyi, float cs, float q, uint32_t sidx) {
                 const int p = pos & (kTcFifo - 1), o = 4 * (p >> 1) + (p & 1);
@@ -361,64 +373,80 @@ conv_mc_tc_f32(const McTcArgs m) {
                 while (tab_end[cur] <= i) ++cur;
                 return ldg_rec(tab_base[cur], i);
             };
+            // `cnt` candidates have been written into FIFO group gi: the writer of the last ones publishes the group
+            auto group_done = [&](int gi, int cnt) {
+                __threadfence_block();
+                const int slot = gi % kTcGroups;
+                if (atomicAdd(s_gcnt + slot, cnt) + cnt == kTcSC) {
+                    s_gcnt[slot] = 0;
+                    __threadfence_block();
+                    grp_n[slot] = (uint32_t)kTcSC;
+                    mbar_arrive(b_cfull + 8 * slot);
+                }
+            };
 
-            PROF_DECL(4);
-            int gpos = 0, published = 0;                              // candidates kept so far (FIFO position, unwrapped); groups published
+            PROF_DECL(8);
+            int blk0 = 0;                                             // blocks of the passes before this one
             for (int pass = 0; rmin + pass * kTcRings <= rmax; ++pass) {
-                // ---- ring table of this pass: lane l of sub-pass t <-> ring number 32 t + l
-                int run = 0;
-                for (int t = 0; t < kTcRings / 32; ++t) {
-                    const int ro = pass * kTcRings + 32 * t + lane;
-                    const int r = flip ? rmax - ro : rmin + ro;
-                    int sa = 0, sn = 0;
-                    if (r >= rmin && r <= rmax) {
-                        int jlo = 0x7fffffff, jhi = -1;
-                        for (int j = 0; j < nrows; ++j) {
-                            const int4 r0 = __ldg((const int4*)(a.rows + row0 + j));
-                            const int k = r - r0.y;
-                            if (k >= 0 && k < r0.z) {
-                                const float4 w = __ldg((const float4*)(a.wins + (size_t)(row0 + j) * a.kmax + k));
-                                const int fl = __float_as_int(w.w);
-                                if (fl == 1) {
-                                    jlo = min(jlo, __float2int_rd(fmaf(fxw, w.z, w.x)));
-                                    jhi = max(jhi, __float2int_rd(fmaf(fxe, w.z, w.y)));
-                                } else if (fl == 2) {
-                                    jlo = 0; jhi = a.m - 1;
+                // ---- ring table of this pass (warp 0): lane l of sub-pass t <-> ring number 32 t + l
+                if (sw == 0) {
+                    int run = 0;
+                    for (int t = 0; t < kTcRings / 32; ++t) {
+                        const int ro = pass * kTcRings + 32 * t + lane;
+                        const int r = flip ? rmax - ro : rmin + ro;
+                        int sa = 0, sn = 0;
+                        if (r >= rmin && r <= rmax) {
+                            int jlo = 0x7fffffff, jhi = -1;
+                            for (int j = 0; j < nrows; ++j) {
+                                const int4 r0 = __ldg((const int4*)(a.rows + row0 + j));
+                                const int k = r - r0.y;
+                                if (k >= 0 && k < r0.z) {
+                                    const float4 w = __ldg((const float4*)(a.wins + (size_t)(row0 + j) * a.kmax + k));
+                                    const int fl = __float_as_int(w.w);
+                                    if (fl == 1) {
+                                        jlo = min(jlo, __float2int_rd(fmaf(fxw, w.z, w.x)));
+                                        jhi = max(jhi, __float2int_rd(fmaf(fxe, w.z, w.y)));
+                                    } else if (fl == 2) {
+                                        jlo = 0; jhi = a.m - 1;
+                                    }
                                 }
                             }
+                            jlo = max(jlo, 0);
+                            jhi = min(jhi, a.m - 1);
+                            if (jhi >= jlo) {
+                                const int32_t* bs = a.bin_start + (size_t)r * a.m;
+                                sa = __ldg(bs + jlo);
+                                sn = __ldg(bs + jhi + 1) - sa;
+                            }
                         }
-                        jlo = max(jlo, 0);
-                        jhi = min(jhi, a.m - 1);
-                        if (jhi >= jlo) {
-                            const int32_t* bs = a.bin_start + (size_t)r * a.m;
-                            sa = __ldg(bs + jlo);
-                            sn = __ldg(bs + jhi + 1) - sa;
-                        }
-                    }
-                    int incl = sn;
+                        int incl = sn;
 #pragma unroll
-                    for (int o = 1; o < 32; o <<= 1) {
-                        const int v = __shfl_up_sync(0xffffffffu, incl, o);
-                        if (lane >= o) incl += v;
+                        for (int o = 1; o < 32; o <<= 1) {
+                            const int v = __shfl_up_sync(0xffffffffu, incl, o);
+                            if (lane >= o) incl += v;
+                        }
+                        incl += run;
+                        tab_end[32 * t + lane] = incl;
+                        tab_base[32 * t + lane] = (unsigned long long)(uintptr_t)(rec + ((long long)sa - (incl - sn)));
+                        run = __shfl_sync(0xffffffffu, incl, 31);
                     }
-                    incl += run;
-                    tab_end[32 * t + lane] = incl;
-                    tab_base[32 * t + lane] = (unsigned long long)(uintptr_t)(rec + ((long long)sa - (incl - sn)));
-                    run = __shfl_sync(0xffffffffu, incl, 31);
                 }
-                __syncwarp();
-                const int total = run;
-                // ---- the stream of this pass in blocks of 32, the records of the next three blocks in flight
+                bar_stream();
+                const int total = tab_end[kTcRings - 1];
+                const int nb = (total + 31) >> 5;
+                PROF_LAP(3);
+                // ---- this warp's blocks of the pass, the records of its next three blocks in flight
                 int cur = 0;
-                uint4 n0 = fetch(lane, total, cur), n1 = fetch(32 + lane, total, cur), n2 = fetch(64 + lane, total, cur);
-                for (int base = 0; base < total; base += 32) {
+                uint4 n0 = fetch(32 * sw + lane, total, cur), n1 = fetch(32 * (sw + kTcSW) + lane, total, cur),
+                      n2 = fetch(32 * (sw + 2 * kTcSW) + lane, total, cur);
+                for (int b = sw; b < nb; b += kTcSW) {
                     const uint4 raw = n0;
                     n0 = n1; n1 = n2;
-                    n2 = fetch(base + 96 + lane, total, cur);
+                    n2 = fetch(32 * (b + 3 * kTcSW) + lane, total, cur);
                     bool keep = false;
                     float cs = 0.f;
                     const int dxi = (int)(raw.x - xc0), dyi = (int)(raw.y - yc0);
-                    if (base + lane < total) {
+                    if (32 * b + lane < total) {
                         const float X = (float)dxi * sxk, Y = (float)dyi * syk;
                         cs = fmaf(Y, fmaf(Y, fmaf(Y, p3, p2), p1), cc0);
                         const float ex = fmaxf(fmaxf(xlo - X, X - xhi), 0.0f), ey = fmaxf(fmaxf(ylo - Y, Y - yhi), 0.0f);
@@ -428,38 +456,52 @@ conv_mc_tc_f32(const McTcArgs m) {
                     }
                     const unsigned mk = __ballot_sync(0xffffffffu, keep);
                     const int nk = __popc(mk);
-                    if (nk == 0) continue;
                     PROF_LAP(0);
-                    // groups this block writes into for the first time must have been released by their readers
-                    const int g_first = (gpos + kTcSC - 1) / kTcSC, g_last = (gpos + nk - 1) / kTcSC;
-                    for (int gi = g_first; gi <= g_last; ++gi)
-                        if (gi >= kTcGroups) mbar_wait(b_cempty + 8 * (gi % kTcGroups), (uint32_t)(gi / kTcGroups - 1) & 1u);
+                    // the token: FIFO position of this block's first candidate, in block order
+                    int gpos = 0;
+                    if (lane == 0) {
+                        while (s_tok[0] != blk0 + b) { }
+                        __threadfence_block();
+                        gpos = s_tok[1];
+                        s_tok[1] = gpos + nk;
+                        __threadfence_block();
+                        s_tok[0] = blk0 + b + 1;
+                    }
+                    gpos = __shfl_sync(0xffffffffu, gpos, 0);
                     PROF_LAP(1);
+                    if (nk == 0) continue;
+                    // the groups this block writes into must have been released by the readers of their previous contents
+                    // (a group's first writer may be another warp that is still waiting for just that)
+                    for (int gi = gpos / kTcSC; gi <= (gpos + nk - 1) / kTcSC; ++gi)
+                        if (gi >= kTcGroups) mbar_wait(b_cempty + 8 * (gi % kTcGroups), (uint32_t)(gi / kTcGroups - 1) & 1u);
+                    PROF_LAP(4);
                     if (keep) put(gpos + __popc(mk & ((1u << lane) - 1u)), dxi, dyi, cs, __uint_as_float(raw.w), raw.z);
                     __syncwarp();
-                    gpos += nk;
-                    // publish the complete groups that are known not to be the last one (a later candidate exists)
-                    const int p_end = (gpos - 1) / kTcSC;
-                    if (lane == 0)
-                        for (int gi = published; gi < p_end; ++gi) {
-                            grp_n[gi % kTcGroups] = (uint32_t)kTcSC;
-                            mbar_arrive(b_cfull + 8 * (gi % kTcGroups));
-                        }
-                    published = max(published, p_end);
+                    if (lane == 0) {
+                        const int ga = gpos / kTcSC, gb = (gpos + nk - 1) / kTcSC;   // nk <= 32: at most two groups
+                        if (ga == gb) group_done(ga, nk);
+                        else { group_done(ga, kTcSC * gb - gpos); group_done(gb, gpos + nk - kTcSC * gb); }
+                    }
+                    PROF_LAP(2);
                 }
+                bar_stream();                                         // every block of the pass has been appended
+                blk0 += nb;
             }
 #ifdef HCG_TC_PROF
-            if (PROF_ON) printf("STREAM: kept %d total %lld | work %lld wait_cempty %lld\n", gpos, clock64() - prof_t0_, prof_[0], prof_[1]);
+            if (PROF_ON && sw == 0) printf("STREAM: kept %d total %lld | fetch+test %lld token %lld wait_cempty %lld put+publish %lld table %lld\n", s_tok[1], clock64() - prof_t0_, prof_[0], prof_[1], prof_[4], prof_[2], prof_[3]);
 #endif
-            // ---- the last group (1 .. kTcSC candidates; none at all: an empty group 0) carries the end-of-tile mark;
-            // its unused slots are filled with candidates far outside every cell's reach (weight 0, never counted)
-            {
-                const int gi = gpos > 0 ? (gpos - 1) / kTcSC : 0;
-                const int nlast = gpos - kTcSC * gi;
+            // ---- the end-of-tile mark: the last, partial group (its unused slots filled with candidates far outside every
+            // cell's reach: weight 0, never counted), or an empty group when the stream ended on a group boundary
+            if (sw == 0) {
+                const int gpos = s_tok[1];
+                const int gi = gpos / kTcSC, nlast = gpos - kTcSC * gi;
+                if (nlast == 0 && gi >= kTcGroups) mbar_wait(b_cempty + 8 * (gi % kTcGroups), (uint32_t)(gi / kTcGroups - 1) & 1u);
                 const int far = __float2int_rn((8.0f * fabsf(a.dyk) + 10.0f * sqrtf(a.hmax)) / syk);
-                if (gpos > 0 && lane >= nlast) put(kTcSC * gi + lane, 0, far, 1.0f, 0.0f, 0u);
+                if (nlast > 0 && lane >= nlast) put(kTcSC * gi + lane, 0, far, 1.0f, 0.0f, 0u);
                 __syncwarp();
                 if (lane == 0) {
+                    s_gcnt[gi % kTcGroups] = 0;
+                    __threadfence_block();
                     grp_n[gi % kTcGroups] = (uint32_t)nlast | 0x80u;
                     mbar_arrive(b_cfull + 8 * (gi % kTcGroups));
                 }
@@ -468,6 +510,9 @@ conv_mc_tc_f32(const McTcArgs m) {
     } else if (warp >= kTcCW) {
         // ================================================================ spectrum rows (B): 128 threads
         asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+        // (Measured and not kept: TMA tile::gather4 requests of 4 rows x 128 bytes land in exactly this layout with
+        // CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B, but the copy engine takes ~47 cycles per request per SM -- 3 x slower
+        // than the 16-byte cp.async below.)
         // thread t4: 16-byte unit u = t4 & 63 of the rows r = 2 i + (t4 >> 6), i = 0 .. kTcSC / 2 - 1, of every stage
         const int t4 = tid - kTcCT;
         const int u = t4 & 63, rp = t4 >> 6;
@@ -618,6 +663,7 @@ conv_mc_tc_f32(const McTcArgs m) {
         };
 
         int k = 0, jd = 0, nst = 0x7fffffff;
+        bool term = false;
         PROF_DECL(8);
         for (;;) {
             if (k >= nst) break;                                     // the last group has been seen
@@ -627,11 +673,14 @@ conv_mc_tc_f32(const McTcArgs m) {
                 PROF_LAP(0); drain(jd); ++jd; PROF_LAP(5);
             }
             PROF_LAP(0);
+#ifdef HCG_TC_PROF
+            if (!mbar_test(b_cfull + 8 * (k % kTcGroups), (uint32_t)(k / kTcGroups) & 1u)) prof_[7] += 1;
+#endif
             mbar_wait(b_cfull + 8 * (k % kTcGroups), (uint32_t)(k / kTcGroups) & 1u);
             PROF_LAP(1);
             const uint32_t info = lds_u1(grp_n_s + 4u * (uint32_t)(k % kTcGroups));
             if (info & 0x80u) nst = (info & 0x7fu) > 0 ? k + 1 : k;
-            if (k >= nst) break;
+            if (k >= nst) { term = true; break; }                   // an empty last group: the stream ended on a group boundary
             const int slot = k % kTcNS;
             if (k >= kTcNS) {
                 mbar_wait(b_empty + 8 * slot, (uint32_t)(k / kTcNS - 1) & 1u);
@@ -696,13 +745,15 @@ conv_mc_tc_f32(const McTcArgs m) {
             ++k;
         }
 #ifdef HCG_TC_PROF
-        if (PROF_ON && warp == 0) printf("COMPUTE: stages %d total %lld | misc %lld wait_cfull %lld wait_empty %lld agen %lld wait_st %lld fence+arrive %lld drain %lld\n",
-                                        k, clock64() - prof_t0_, prof_[0], prof_[1], prof_[2], prof_[3], prof_[4], prof_[6], prof_[5]);
+        if (PROF_ON && warp == 0) printf("COMPUTE: stages %d total %lld | misc %lld wait_cfull %lld (not ready %lld times) wait_empty %lld agen %lld wait_st %lld fence+arrive %lld drain %lld\n",
+                                        k, clock64() - prof_t0_, prof_[0], prof_[1], prof_[7], prof_[2], prof_[3], prof_[4], prof_[6], prof_[5]);
 #endif
-        if (nst == 0) {                                              // nothing can reach this tile: release the MMA warp
-            if (tid == 0) s_flag[0] = 3u;
+        if (term) {                                                  // no stage carried the end-of-tile mark: send it on its own
+            const int slot = nst % kTcNS;
+            if (nst >= kTcNS) mbar_wait(b_empty + 8 * slot, (uint32_t)(nst / kTcNS - 1) & 1u);
+            if (tid == 0) s_flag[slot] = 3u;
             __syncwarp();
-            if (lane == 0) mbar_arrive(b_afull);
+            if (lane == 0) mbar_arrive(b_afull + 8 * slot);
         }
         for (const int nchunk = (nst + kTcCH - 1) / kTcCH; jd < nchunk; ++jd) drain(jd);
 
