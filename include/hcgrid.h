@@ -90,11 +90,15 @@ typedef struct {
     float us_pixelise, us_sort, us_tables, us_pack, us_convolve, us_total; /* PROFILE only   */
     int32_t split;            /* warps per tile used (tile kernel; else 1)                    */
     int32_t preorder;         /* pre-ordering used: 1 radix sort, 2 counting sort             */
+    int64_t n_hit;            /* PROFILE + count output: pairs (cell, sample) with d <= R = sum of the counts
+                                 ("kernel evaluations"); -1 otherwise                            */
+    int64_t n_pairs_tested;   /* PROFILE, tile kernel: pairs the kernel put to the distance test (candidate
+                                 stream length x cells of every tile); -1 otherwise                           */
 } hcgrid_stats;
 
 /* Create a context.  sigma_deg = kernel standard deviation, support_radius_deg =
  * "sphere_radius", nside = HEALPix partition level N_side,
- * a power of two in [1, 8192].  precision = HCGRID_F32 or HCGRID_F64.  device = CUDA
+ * a power of two in [1, 16384] (12 nside^2 <= 2^32: the pixel index fits the sort key).  precision = HCGRID_F32 or HCGRID_F64.  device = CUDA
  * ordinal.  On failure *out is NULL and the message is available through
  * hcgrid_last_error(NULL). */
 int hcgrid_create(hcgrid_ctx** out, double sigma_deg, double support_radius_deg,

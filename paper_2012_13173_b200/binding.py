@@ -46,7 +46,8 @@ class Stats(ctypes.Structure):
                 ("kernel", ctypes.c_int32), ("gpu_launches", ctypes.c_int32), ("coarsen_y", ctypes.c_int32),
                 ("us_pixelise", ctypes.c_float), ("us_sort", ctypes.c_float), ("us_tables", ctypes.c_float),
                 ("us_pack", ctypes.c_float), ("us_convolve", ctypes.c_float), ("us_total", ctypes.c_float),
-                ("split", ctypes.c_int32), ("preorder", ctypes.c_int32)]
+                ("split", ctypes.c_int32), ("preorder", ctypes.c_int32),
+                ("n_hit", ctypes.c_int64), ("n_pairs_tested", ctypes.c_int64)]
 
     def asdict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

@@ -44,8 +44,8 @@ int hcgrid_create(hcgrid_ctx** out, double sigma_deg, double support_radius_deg,
         return fail(nullptr, HCGRID_ERR_INVALID_ARG, "sigma_deg must be a positive finite number");
     if (!(support_radius_deg > 0.0) || !(support_radius_deg < 90.0))
         return fail(nullptr, HCGRID_ERR_INVALID_ARG, "support_radius_deg must be in (0, 90)");
-    if (!is_pow2(nside) || nside > 8192)
-        return fail(nullptr, HCGRID_ERR_INVALID_ARG, "nside must be a power of two in [1, 8192]");
+    if (!is_pow2(nside) || nside > 16384)
+        return fail(nullptr, HCGRID_ERR_INVALID_ARG, "nside must be a power of two in [1, 16384]");
     if (precision != HCGRID_F32 && precision != HCGRID_F64)
         return fail(nullptr, HCGRID_ERR_INVALID_ARG, "precision must be HCGRID_F32 or HCGRID_F64");
     int ndev = 0;
@@ -85,7 +85,7 @@ int hcgrid_destroy(hcgrid_ctx* c) {
     if (!c) return HCGRID_OK;
     cudaSetDevice(c->device);
     DevBuf* bufs[] = {&c->d_strips, &c->d_wins, &c->d_winsf, &c->d_rowsf, &c->d_cell_lon, &c->d_cell_lat, &c->d_keys, &c->d_keys_out,
-                      &c->d_idx, &c->d_idx_out, &c->d_sort_tmp, &c->d_bins, &c->d_rec, &c->d_misc, &c->d_long, &c->d_dirty,
+                      &c->d_idx, &c->d_idx_out, &c->d_sort_tmp, &c->d_bins, &c->d_rec, &c->d_misc, &c->d_long, &c->d_dirty, &c->d_stat,
                       &c->d_in_lon, &c->d_in_lat, &c->d_in_val, &c->d_in_wgt, &c->d_out_cube, &c->d_out_w,
                       &c->d_out_cnt, &c->d_acc_cube, &c->d_acc_w, &c->d_acc_cnt, &c->d_tmp_cube, &c->d_tmp_w,
                       &c->d_tmp_cnt};
@@ -206,6 +206,8 @@ int hcgrid_grid(hcgrid_ctx* c, int64_t n, const double* lon, const double* lat, 
     rc = run_convolve(c, n, values, nchan, weights != nullptr, cube, wmap, counts, st);
     if (rc != HCGRID_OK) return rc;
     if (c->opt_profile) { cudaEventRecord(c->ev[5], st); c->ev_valid = true; }
+    rc = run_profile_stats(c, counts, st);
+    if (rc != HCGRID_OK) return rc;
     c->stats.n_kept = -1;   // resolved lazily by hcgrid_get_stats
     return HCGRID_OK;
 }
@@ -311,6 +313,15 @@ int hcgrid_get_stats(const hcgrid_ctx* cc, hcgrid_stats* out) {
         float ms = 0.f;
         HCG_CUDA(c, cudaEventElapsedTime(&ms, c->ev[0], c->ev[5]));
         c->stats.us_total = ms * 1000.f;
+    }
+    c->stats.n_hit = -1;
+    c->stats.n_pairs_tested = -1;
+    if (c->stat_hit || c->stat_pairs) {
+        HCG_CUDA(c, cudaStreamSynchronize(c->last_stream));
+        long long v[2] = {0, 0};
+        HCG_CUDA(c, cudaMemcpy(v, c->d_stat.p, 16, cudaMemcpyDeviceToHost));
+        if (c->stat_hit) c->stats.n_hit = v[0];
+        if (c->stat_pairs) c->stats.n_pairs_tested = v[1];
     }
     c->stats.n_bins = c->region.nbins;
     c->stats.n_rings = c->region.nring;

@@ -281,6 +281,35 @@ static int launch_f32(hcgrid_ctx* c, ConvArgs& a, bool hasq, bool staged, cudaSt
     return HCGRID_OK;
 }
 
+// n_hit of hcgrid_stats: the sum of the count output (profiling only)
+__global__ void __launch_bounds__(256) sum_counts_kernel(const int32_t* __restrict__ counts, int64_t ncell, unsigned long long* out) {
+    long long s = 0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < ncell; i += (int64_t)gridDim.x * blockDim.x) s += counts[i];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0 && s != 0) atomicAdd(out, (unsigned long long)s);   // integer: order-independent
+}
+
+// The profiling-only figures of hcgrid_stats, after the timed stages: n_hit (sum of the count output) and, for the tile
+// kernel, n_pairs_tested.
+int run_profile_stats(hcgrid_ctx* c, int32_t* counts, cudaStream_t st) {
+    c->stat_hit = c->stat_pairs = false;
+    if (!c->opt_profile) return HCGRID_OK;
+    HCG_CUDA(c, c->d_stat.ensure(16));
+    HCG_CUDA(c, cudaMemsetAsync(c->d_stat.p, 0, 16, st));
+    if (counts && !c->raw_sums) {
+        sum_counts_kernel<<<4 * c->num_sms, 256, 0, st>>>(counts, c->ncell, c->d_stat.as<unsigned long long>());
+        HCG_CUDA(c, cudaGetLastError());
+        c->stat_hit = true;
+    }
+    if (c->stats.kernel == 6) {
+        const int rc = launch_tile_pairs_tested(c, c->stats.coarsen, c->stats.coarsen_y, c->d_stat.as<unsigned long long>() + 1, st);
+        if (rc != HCGRID_OK) return rc;
+        c->stat_pairs = true;
+    }
+    return HCGRID_OK;
+}
+
 int run_convolve(hcgrid_ctx* c, int64_t n, const float* values, int nchan, bool has_weights, void* cube,
                  void* wmap, int32_t* counts, cudaStream_t st) {
     const Region& rg = c->region;

@@ -147,14 +147,6 @@ __device__ __forceinline__ uint32_t lds_u1(uint32_t addr) {
 __device__ __forceinline__ void sts_u4(uint32_t addr, uint4 v) {
     asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
-#ifdef HCG_TC_PROF
-#define PROF_DECL(n) long long prof_[n] = {}; long long prof_t_ = clock64(); const long long prof_t0_ = prof_t_; (void)prof_t0_
-#define PROF_LAP(i) do { const long long t_ = clock64(); prof_[i] += t_ - prof_t_; prof_t_ = t_; } while (0)
-#define PROF_ON (blockIdx.x == 300 && blockIdx.y == 0 && lane == 0)
-#else
-#define PROF_DECL(n)
-#define PROF_LAP(i)
-#endif
 // keep a loop-invariant value in its register (ptxas otherwise recomputes it from the thread index every iteration)
 #define HCG_PIN(x) asm volatile("" : "+r"(x))
 
@@ -270,21 +262,16 @@ conv_mc_tc_f32(const McTcArgs m) {
             // ============================================================ MMA issuer (lane 0 issues; the warp stays converged)
             const uint32_t idesc = umma_idesc_tf32(nch);
             const uint64_t b_rw0 = umma_desc(s_base + kOffBraw, 1024, 512, 1), b_lo0 = umma_desc(s_base + kOffBlo, 1024, 512, 1);
-            PROF_DECL(4);
             for (int s = 0;; ++s) {
                 const int slot = s % kTcNS;
                 const uint32_t par = (uint32_t)(s / kTcNS) & 1u;
-                PROF_LAP(0);
                 mbar_wait(b_afull + 8 * slot, par);
-                PROF_LAP(1);
                 const uint32_t flag = s_flag[slot];
                 if (!(flag & 2u)) {
                     mbar_wait(b_bfull + 8 * slot, par);
-                    PROF_LAP(2);
                     const int chunk = s / kTcCH;
                     const bool first = s % kTcCH == 0;
                     if (first && chunk >= 1) mbar_wait(b_dempty, (uint32_t)(chunk - 1) & 1u);   // the previous chunk has been taken over
-                    PROF_LAP(3);
                     tc_fence_after();
                     if (lane == 0) {
                         const uint64_t so = (uint64_t)((uint32_t)slot * (kStageBytes >> 4));
@@ -292,13 +279,9 @@ conv_mc_tc_f32(const McTcArgs m) {
                         for (int ks = 0; ks < kTcKS; ++ks) {
                             const uint32_t ah = tm + kTmemA + (uint32_t)(slot * kTmemAStage + ks * 8), al = ah + 8 * kTcKS;
                             const uint64_t br = b_rw0 + so + (uint64_t)(ks * (8192 >> 4)), bl = b_lo0 + so + (uint64_t)(ks * (8192 >> 4));
-#ifndef HCG_TC_NOMMA
                             umma_tf32_ts(tm, ah, br, idesc, (first && ks == 0) ? 0u : 1u);
                             umma_tf32_ts(tm, al, br, idesc, 1u);
                             umma_tf32_ts(tm, ah, bl, idesc, 1u);
-#else
-                            (void)ah; (void)al; (void)br; (void)bl;
-#endif
                         }
                         tc_commit(b_empty + 8 * slot);
                         if (s % kTcCH == kTcCH - 1 || (flag & 1u)) tc_commit(b_dfull);
@@ -309,9 +292,6 @@ conv_mc_tc_f32(const McTcArgs m) {
                     __syncwarp();
                 }
                 if (flag & 1u) {
-#ifdef HCG_TC_PROF
-                    if (PROF_ON) printf("MMA: stages %d total %lld | issue+misc %lld wait_afull %lld wait_bfull %lld wait_dempty %lld\n", s + 1, clock64() - prof_t0_, prof_[0], prof_[1], prof_[2], prof_[3]);
-#endif
                     break;
                 }
             }
@@ -385,7 +365,6 @@ conv_mc_tc_f32(const McTcArgs m) {
                 }
             };
 
-            PROF_DECL(8);
             int blk0 = 0;                                             // blocks of the passes before this one
             for (int pass = 0; rmin + pass * kTcRings <= rmax; ++pass) {
                 // ---- ring table of this pass (warp 0): lane l of sub-pass t <-> ring number 32 t + l
@@ -434,7 +413,6 @@ conv_mc_tc_f32(const McTcArgs m) {
                 bar_stream();
                 const int total = tab_end[kTcRings - 1];
                 const int nb = (total + 31) >> 5;
-                PROF_LAP(3);
                 // ---- this warp's blocks of the pass, the records of its next three blocks in flight
                 int cur = 0;
                 uint4 n0 = fetch(32 * sw + lane, total, cur), n1 = fetch(32 * (sw + kTcSW) + lane, total, cur),
@@ -456,7 +434,6 @@ conv_mc_tc_f32(const McTcArgs m) {
                     }
                     const unsigned mk = __ballot_sync(0xffffffffu, keep);
                     const int nk = __popc(mk);
-                    PROF_LAP(0);
                     // the token: FIFO position of this block's first candidate, in block order
                     int gpos = 0;
                     if (lane == 0) {
@@ -468,13 +445,11 @@ conv_mc_tc_f32(const McTcArgs m) {
                         s_tok[0] = blk0 + b + 1;
                     }
                     gpos = __shfl_sync(0xffffffffu, gpos, 0);
-                    PROF_LAP(1);
                     if (nk == 0) continue;
                     // the groups this block writes into must have been released by the readers of their previous contents
                     // (a group's first writer may be another warp that is still waiting for just that)
                     for (int gi = gpos / kTcSC; gi <= (gpos + nk - 1) / kTcSC; ++gi)
                         if (gi >= kTcGroups) mbar_wait(b_cempty + 8 * (gi % kTcGroups), (uint32_t)(gi / kTcGroups - 1) & 1u);
-                    PROF_LAP(4);
                     if (keep) put(gpos + __popc(mk & ((1u << lane) - 1u)), dxi, dyi, cs, __uint_as_float(raw.w), raw.z);
                     __syncwarp();
                     if (lane == 0) {
@@ -482,14 +457,10 @@ conv_mc_tc_f32(const McTcArgs m) {
                         if (ga == gb) group_done(ga, nk);
                         else { group_done(ga, kTcSC * gb - gpos); group_done(gb, gpos + nk - kTcSC * gb); }
                     }
-                    PROF_LAP(2);
                 }
                 bar_stream();                                         // every block of the pass has been appended
                 blk0 += nb;
             }
-#ifdef HCG_TC_PROF
-            if (PROF_ON && sw == 0) printf("STREAM: kept %d total %lld | fetch+test %lld token %lld wait_cempty %lld put+publish %lld table %lld\n", s_tok[1], clock64() - prof_t0_, prof_[0], prof_[1], prof_[4], prof_[2], prof_[3]);
-#endif
             // ---- the end-of-tile mark: the last, partial group (its unused slots filled with candidates far outside every
             // cell's reach: weight 0, never counted), or an empty group when the stream ended on a group boundary
             if (sw == 0) {
@@ -531,28 +502,20 @@ conv_mc_tc_f32(const McTcArgs m) {
         // row r = 2 i + rp of the stage: (r >> 3) = i >> 2, (r >> 2) & 1 = (i >> 1) & 1, r & 3 = 2 (i & 1) + rp
         auto unit_off = [&](int i) -> uint32_t { return (uint32_t)((i >> 2) * 8192 + ((i >> 1) & 1) * 512) + off_u[i & 1]; };
         constexpr int NU = kTcSC / 2;                                 // units per thread per stage
-        PROF_DECL(8);
         int nst = 0x7fffffff, pf = 0;
         for (int k = 0;; ++k) {
             // request the rows of the stages up to k + BD (the missing rows of the last stage are zeros)
             while (pf <= k + kTcBD) {
                 if (pf < nst) {
                     const int grp = pf % kTcGroups, slot = pf % kTcNS;
-                    PROF_LAP(0);
                     mbar_wait(b_cfull + 8 * grp, (uint32_t)(pf / kTcGroups) & 1u);
-                    PROF_LAP(1);
                     const uint32_t info = lds_u1(grp_n_s + 4u * (uint32_t)grp);
                     const int n = (int)(info & 0x7fu);
                     if (info & 0x80u) nst = n > 0 ? pf + 1 : pf;
                     if (pf < nst) {
                         if (pf >= kTcNS) mbar_wait(b_empty + 8 * slot, (uint32_t)(pf / kTcNS - 1) & 1u);
-                        PROF_LAP(2);
                         const uint32_t sb = s_base + (uint32_t)slot * kStageBytes + kOffBraw;
-#ifdef HCG_TC_NOB
-                        if (false) {
-#else
                         if (on) {
-#endif
 #pragma unroll
                             for (int i0 = 0; i0 < NU; i0 += 8) {
                                 uint32_t idx[8];
@@ -575,16 +538,10 @@ conv_mc_tc_f32(const McTcArgs m) {
             }
             if (k >= nst) break;
             // the rows of stage k have landed (each thread reads back its own bytes): lo = v - trunc_tf32(v)
-            PROF_LAP(0);
             cp_wait<kTcBD>();
-            PROF_LAP(3);
             const int slot = k % kTcNS;
             const uint32_t sb = s_base + (uint32_t)slot * kStageBytes + kOffBraw;
-#ifdef HCG_TC_NOB
-            if (false) {
-#else
             if (on) {
-#endif
 #pragma unroll
                 for (int i0 = 0; i0 < NU; i0 += 4) {
                     uint4 v[4];
@@ -601,16 +558,11 @@ conv_mc_tc_f32(const McTcArgs m) {
                     }
                 }
             }
-            PROF_LAP(4);
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             __syncwarp();
             if (lane == 0) mbar_arrive(b_bfull + 8 * slot);
-            PROF_LAP(5);
         }
         cp_wait<0>();
-#ifdef HCG_TC_PROF
-        if (PROF_ON && warp == kTcCW) printf("BROWS: total %lld | issue %lld wait_cfull %lld wait_empty %lld cp_wait %lld split %lld fence+arrive %lld\n", clock64() - prof_t0_, prof_[0], prof_[1], prof_[2], prof_[3], prof_[4], prof_[5]);
-#endif
     } else {
         // ================================================================ A (kernel weights) and the accumulators
         asm volatile("setmaxnreg.inc.sync.aligned.u32 200;");
@@ -664,20 +616,13 @@ conv_mc_tc_f32(const McTcArgs m) {
 
         int k = 0, jd = 0, nst = 0x7fffffff;
         bool term = false;
-        PROF_DECL(8);
         for (;;) {
             if (k >= nst) break;                                     // the last group has been seen
             // the chunk the MMA warp has finished must be taken over before it can start the next: as soon as it is
             // complete, and at the latest when this warp would have to wait for a stage of the following chunk
-            if (jd < k / kTcCH && (k == (jd + 1) * kTcCH + kTcNS - 1 || mbar_test(b_dfull, (uint32_t)jd & 1u))) {
-                PROF_LAP(0); drain(jd); ++jd; PROF_LAP(5);
+            if (jd < k / kTcCH && (k == (jd + 1) * kTcCH + kTcNS - 1 || mbar_test(b_dfull, (uint32_t)jd & 1u))) { drain(jd); ++jd; 
             }
-            PROF_LAP(0);
-#ifdef HCG_TC_PROF
-            if (!mbar_test(b_cfull + 8 * (k % kTcGroups), (uint32_t)(k / kTcGroups) & 1u)) prof_[7] += 1;
-#endif
             mbar_wait(b_cfull + 8 * (k % kTcGroups), (uint32_t)(k / kTcGroups) & 1u);
-            PROF_LAP(1);
             const uint32_t info = lds_u1(grp_n_s + 4u * (uint32_t)(k % kTcGroups));
             if (info & 0x80u) nst = (info & 0x7fu) > 0 ? k + 1 : k;
             if (k >= nst) { term = true; break; }                   // an empty last group: the stream ended on a group boundary
@@ -686,7 +631,6 @@ conv_mc_tc_f32(const McTcArgs m) {
                 mbar_wait(b_empty + 8 * slot, (uint32_t)(k / kTcNS - 1) & 1u);
                 tc_fence_after();
             }
-            PROF_LAP(2);
 
             // ---- A: K-steps g * kTcKS / 2 .. of the stage x this thread's cell, two candidates per instruction
 #pragma unroll
@@ -731,9 +675,7 @@ conv_mc_tc_f32(const McTcArgs m) {
                 asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
                              ::"r"(t_lo), "r"(lo[0]), "r"(lo[1]), "r"(lo[2]), "r"(lo[3]), "r"(lo[4]), "r"(lo[5]), "r"(lo[6]), "r"(lo[7]) : "memory");
             }
-            PROF_LAP(3);
             tmem_st_wait();
-            PROF_LAP(4);
             tc_fence_before();
             if (tid == 0) s_flag[slot] = k == nst - 1 ? 1u : 0u;
             __syncwarp();
@@ -741,13 +683,8 @@ conv_mc_tc_f32(const McTcArgs m) {
                 mbar_arrive(b_cempty + 8 * (k % kTcGroups));          // this warp is done with the group's FIFO entries
                 mbar_arrive(b_afull + 8 * slot);
             }
-            PROF_LAP(6);
             ++k;
         }
-#ifdef HCG_TC_PROF
-        if (PROF_ON && warp == 0) printf("COMPUTE: stages %d total %lld | misc %lld wait_cfull %lld (not ready %lld times) wait_empty %lld agen %lld wait_st %lld fence+arrive %lld drain %lld\n",
-                                        k, clock64() - prof_t0_, prof_[0], prof_[1], prof_[7], prof_[2], prof_[3], prof_[4], prof_[6], prof_[5]);
-#endif
         if (term) {                                                  // no stage carried the end-of-tile mark: send it on its own
             const int slot = nst % kTcNS;
             if (nst >= kTcNS) mbar_wait(b_empty + 8 * slot, (uint32_t)(nst / kTcNS - 1) & 1u);

@@ -350,4 +350,64 @@ int launch_conv_tile(hcgrid_ctx* c, int64_t n, float* cube, float* wmap, int32_t
     return HCGRID_OK;
 }
 
+// ------------------------------------------------------------------ profiling: pairs put to the distance test
+// One thread per tile: steps (i)-(iii) exactly as conv1_tile_f32 takes them (union of the rows' ring ranges, united
+// lookup-bin windows, two table reads per ring) give the length of the tile's candidate stream; every candidate is
+// tested against every cell of the tile.
+__global__ void __launch_bounds__(256) tile_pairs_tested_kernel(const TileArgs a, int gx, int gy, unsigned long long* out) {
+    const int64_t tile = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long pairs = 0;
+    if (tile < a.ntiles) {
+        const int ty = (int)(tile / a.tiles_x);
+        const int ix0 = (int)(tile - (int64_t)ty * a.tiles_x) * gx, row0 = ty * gy;
+        const int ncols = min(gx, a.nx - ix0), nrows = min(gy, a.ny - row0);
+        int rmin = 0x7fffffff, rmax = -0x7fffffff;
+        for (int j = 0; j < nrows; ++j) {
+            const int4 r0 = __ldg((const int4*)(a.rows + row0 + j));
+            rmin = min(rmin, r0.y);
+            rmax = max(rmax, r0.y + r0.z - 1);
+        }
+        const float fxw = (float)(a.du >= 0.0 ? ix0 : ix0 + ncols - 1), fxe = (float)(a.du >= 0.0 ? ix0 + ncols - 1 : ix0);
+        long long total = 0;
+        for (int r = rmin; r <= rmax; ++r) {
+            int jlo = 0x7fffffff, jhi = -1;
+            for (int j = 0; j < nrows; ++j) {
+                const int4 r0 = __ldg((const int4*)(a.rows + row0 + j));
+                const int k = r - r0.y;
+                if (k >= 0 && k < r0.z) {
+                    const float4 w = __ldg((const float4*)(a.wins + (size_t)(row0 + j) * a.kmax + k));
+                    const int fl = __float_as_int(w.w);
+                    if (fl == 1) {
+                        jlo = min(jlo, __float2int_rd(fmaf(fxw, w.z, w.x)));
+                        jhi = max(jhi, __float2int_rd(fmaf(fxe, w.z, w.y)));
+                    } else if (fl == 2) {
+                        jlo = 0; jhi = a.m - 1;
+                    }
+                }
+            }
+            jlo = max(jlo, 0);
+            jhi = min(jhi, a.m - 1);
+            if (jhi >= jlo) {
+                const int32_t* bs = a.bin_start + (size_t)r * a.m;
+                total += __ldg(bs + jhi + 1) - __ldg(bs + jlo);
+            }
+        }
+        pairs = (unsigned long long)total * (unsigned long long)(ncols * nrows);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) pairs += __shfl_xor_sync(0xffffffffu, pairs, o);
+    if ((threadIdx.x & 31) == 0 && pairs != 0) atomicAdd(out, pairs);   // integer: order-independent
+}
+
+int launch_tile_pairs_tested(hcgrid_ctx* c, int gx, int gy, unsigned long long* out, cudaStream_t st) {
+    TileArgs a{};
+    fill_tile_args(c, tile_series_mode(c), a);
+    a.tiles_x = (a.nx + gx - 1) / gx;
+    a.ntiles = (int64_t)a.tiles_x * ((a.ny + gy - 1) / gy);
+    tile_pairs_tested_kernel<<<(unsigned)((a.ntiles + 255) / 256), 256, 0, st>>>(a, gx, gy, out);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e, "tile_pairs_tested_kernel");
+    return HCGRID_OK;
+}
+
 }  // namespace hcg

@@ -151,7 +151,7 @@ struct hcgrid_ctx {
     double dlmax = 0.0;                  // widest longitude half-window of a support disc, rad
     bool tile_ok = false;                // the tile kernel's preconditions hold for this target
     // per-call scratch
-    hcg::DevBuf d_keys, d_keys_out, d_idx, d_idx_out, d_sort_tmp, d_bins, d_rec, d_misc, d_long, d_dirty;
+    hcg::DevBuf d_keys, d_keys_out, d_idx, d_idx_out, d_sort_tmp, d_bins, d_rec, d_misc, d_long, d_dirty, d_stat;
     hcg::DevBuf d_in_lon, d_in_lat, d_in_val, d_in_wgt, d_out_cube, d_out_w, d_out_cnt;  // *_host path
     // incremental gridding (hcgrid_accumulate / hcgrid_finalize): un-normalised sums over the batches so far
     hcg::DevBuf d_acc_cube, d_acc_w, d_acc_cnt, d_tmp_cube, d_tmp_w, d_tmp_cnt;
@@ -168,6 +168,7 @@ struct hcgrid_ctx {
     int opt_host_chunks = 0;
     cudaEvent_t ev[8] = {};
     bool ev_valid = false;
+    bool stat_hit = false, stat_pairs = false;   // d_stat[0] / d_stat[1] hold n_hit / n_pairs_tested of the last call
     hcgrid_stats stats{};
     std::string err;
 };
@@ -181,6 +182,8 @@ int run_preorder(hcgrid_ctx* c, int64_t n, const double* lon, const double* lat,
                  int nchan, const float* weights, cudaStream_t st);
 int run_convolve(hcgrid_ctx* c, int64_t n, const float* values, int nchan, bool has_weights,
                  void* cube, void* wmap, int32_t* counts, cudaStream_t st);
+
+int run_profile_stats(hcgrid_ctx* c, int32_t* counts, cudaStream_t st);
 
 int fail(hcgrid_ctx* c, int code, const char* fmt, ...);
 int cuda_fail(hcgrid_ctx* c, cudaError_t e, const char* what);

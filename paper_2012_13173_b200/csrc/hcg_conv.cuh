@@ -99,6 +99,9 @@ __device__ __forceinline__ bool pair32(const Rec32& r, const TaskConst& tc, floa
 // launcher of convolve_tile.cu (single channel, fp32, plate-carree targets)
 int launch_conv_tile(hcgrid_ctx* c, int64_t n, float* cube, float* wmap, int32_t* counts, cudaStream_t st);
 
+// pairs the tile kernel puts to the distance test with gx x gy tiles: candidate-stream length x cells of every tile, added to *out
+int launch_tile_pairs_tested(hcgrid_ctx* c, int gx, int gy, unsigned long long* out, cudaStream_t st);
+
 // launcher of convolve_mc.cu (many channels, fp32, plate-carree targets, nchan % 4 == 0)
 int launch_conv_mc(hcgrid_ctx* c, const float* values, int nchan, float* cube, float* wmap, int32_t* counts,
                    cudaStream_t st);

@@ -365,7 +365,7 @@ def test_full_size_sampled_cells(oracle, cfg, k):
     cube, wmap, cnt, st = run_gpu(w, "f32")          # default options, with the count output
     r = compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F32, qmax(w), cells=cells)
     assert r["n_hit"] > 0
-    assert st["kernel"] == (7 if cfg == 4 else 6)
+    assert st["kernel"] == (8 if cfg == 4 else 6)     # config 4: the tensor-core cube kernel
     # exactly what bench.py times: default options, datacube + weight map only (no count output)
     cube_b, wmap_b, none, st_b = run_gpu(w, "f32", want_counts=False)
     assert none is None and st_b["kernel"] == st["kernel"]
