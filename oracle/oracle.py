@@ -66,6 +66,7 @@ class OracleResult:
     near_boundary: np.ndarray  # [ncell] int64: pairs with |d - R| < 1e-9 rad
     threads: int
     abswmap: np.ndarray = None  # [ncell] float64: sum |q w| (kernel= calls only)
+    vmax: float = 1.0           # largest |value| of the input (finite ones): scale of a boundary pair's effect on V
 
 
 def _ptr(a):
@@ -73,6 +74,11 @@ def _ptr(a):
 
 
 GAUSS, TAPERED_SINC = 0, 1
+
+
+def _vmax(values) -> float:
+    a = np.abs(values[np.isfinite(values)]) if values.size else values
+    return float(a.max()) if a.size else 0.0
 
 
 def grid(sigma_deg, radius_deg, cell_lon, cell_lat, lon, lat, values, weights=None,
@@ -112,14 +118,14 @@ def grid(sigma_deg, radius_deg, cell_lon, cell_lat, lon, lat, values, weights=No
                                            _ptr(counts), _ptr(absmap), _ptr(absw), _ptr(nb), int(nthreads))
         if rc != 0:
             raise ValueError("hcgrid_oracle_grid_kernel rejected its arguments")
-        return OracleResult(cube, wmap, counts, absmap, nb, int(lib.hcgrid_oracle_last_threads()), absw)
+        return OracleResult(cube, wmap, counts, absmap, nb, int(lib.hcgrid_oracle_last_threads()), absw, _vmax(values))
     rc = lib.hcgrid_oracle_grid(float(sigma_deg), float(radius_deg), ncell, _ptr(cell_lon),
                                 _ptr(cell_lat), n, _ptr(lon), _ptr(lat), _ptr(values), nchan,
                                 _ptr(weights), _ptr(cube), _ptr(wmap), _ptr(counts),
                                 _ptr(absmap), _ptr(nb), int(nthreads))
     if rc != 0:
         raise ValueError("hcgrid_oracle_grid rejected its arguments")
-    return OracleResult(cube, wmap, counts, absmap, nb, int(lib.hcgrid_oracle_last_threads()))
+    return OracleResult(cube, wmap, counts, absmap, nb, int(lib.hcgrid_oracle_last_threads()), None, _vmax(values))
 
 
 if __name__ == "__main__":
