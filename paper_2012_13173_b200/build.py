@@ -26,15 +26,33 @@ def _nvcc() -> str:
     raise RuntimeError("nvcc not found: the CUDA library cannot be built")
 
 
-def _deps_mtime() -> float:
-    paths = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(INCLUDE, "hcgrid.h")]
-    return max(os.path.getmtime(p) for p in paths)
+HASH = LIB + ".srchash"
+
+
+def source_hash() -> str:
+    """sha256 over csrc/* and include/hcgrid.h (names and contents) and the compiler flags: the library is
+    rebuilt whenever this differs from the hash stored beside it (modification times tie after a fresh checkout)."""
+    import hashlib
+    h = hashlib.sha256(" ".join(NVCC_FLAGS).encode())
+    for path in sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC)) + [os.path.join(INCLUDE, "hcgrid.h")]:
+        h.update(os.path.basename(path).encode())
+        with open(path, "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()
+
+
+def _stored_hash() -> str:
+    try:
+        with open(HASH) as fh:
+            return fh.read().strip()
+    except OSError:
+        return ""
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
     """Compile every csrc/*.cu for sm_100a and link libhcgrid.so.  Returns its path."""
-    newest = _deps_mtime()
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
+    want = source_hash()
+    if not force and os.path.exists(LIB) and _stored_hash() == want:
         return LIB
     nvcc = _nvcc()
     os.makedirs(OBJ, exist_ok=True)
@@ -62,6 +80,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
+    with open(HASH, "w") as fh:
+        fh.write(want + "\n")
     return LIB
 
 

@@ -7,7 +7,7 @@
 //   north cap  (i <  nside):        4 i pixels, centre z = 1 - i^2 / (3 nside^2)
 //   belt       (nside <= i <= 3n):  4 nside pixels, centre z = (2 nside - i) * 2 / (3 nside)
 //   south cap  by mirror symmetry (i' = 4 nside - i).
-// Two containment facts the gather relies on (tests/test_healpix.py checks both):
+// Two containment facts the gather relies on (tests/test_library_cpu.py checks both):
 //   (1) a point assigned to pixel j of ring r satisfies j <= g_r(lon) <= j+1 with
 //       g_r(lon) = lon * npix_ring(r) / (2 pi) + off_r   (off_r = 1/2 on belt rings whose
 //       pixel centres sit at multiples of the pixel width, else 0);
