@@ -92,8 +92,8 @@ typedef struct {
     int32_t preorder;         /* pre-ordering used: 1 radix sort, 2 counting sort             */
     int64_t n_hit;            /* PROFILE + count output: pairs (cell, sample) with d <= R = sum of the counts
                                  ("kernel evaluations"); -1 otherwise                            */
-    int64_t n_pairs_tested;   /* PROFILE, tile kernel: pairs the kernel put to the distance test (candidate
-                                 stream length x cells of every tile); -1 otherwise                           */
+    int64_t n_pairs_tested;   /* PROFILE, tile and strip kernels (kernel 1..6): pairs the kernel put to the distance
+                                 test (candidate stream length x cells of every tile or task); -1 otherwise     */
 } hcgrid_stats;
 
 /* Create a context.  sigma_deg = kernel standard deviation, support_radius_deg =

@@ -98,13 +98,17 @@ conv1_simple_f32(const ConvArgs a) {
     for (int g = 0; g < G; ++g) { acc.W[g] = 0.f; acc.S[g] = 0.f; acc.cnt[g] = 0; }
     for (int k = 0; k < st.nring; ++k) {
         const RingWin w = a.wins[(size_t)s * a.kmax + k];
-        int sa, sn;
-        ring_segment(w, ix0, ncells, a.rg, a.bin_start, sa, sn);
-        for (int i = lane; i < sn; i += 32) {
-            const uint4 raw = __ldg((const uint4*)(rec + sa + i));
-            Rec32 r;
-            r.xi = raw.x; r.yi = raw.y; r.idx = raw.z; r.q = __uint_as_float(raw.w);
-            pair_update<G, HASQ>(r, tc, acc);
+        int sa, sn, sa2, sn2;
+        ring_segment(w, ix0, ncells, a.rg, a.bin_start, sa, sn, sa2, sn2);
+        for (int seg = 0; seg < 2; ++seg) {
+            for (int i = lane; i < sn; i += 32) {
+                const uint4 raw = __ldg((const uint4*)(rec + sa + i));
+                Rec32 r;
+                r.xi = raw.x; r.yi = raw.y; r.idx = raw.z; r.q = __uint_as_float(raw.w);
+                pair_update<G, HASQ>(r, tc, acc);
+            }
+            sa = sa2; sn = sn2;     // second range: only where the window crosses the seam of a full-circle region
+            if (sn == 0) break;
         }
     }
     task_finish<G>(acc, lane, (int64_t)s * a.strip_cells + ix0, ncells, (float*)a.cube, (float*)a.wmap, a.counts);
@@ -290,8 +294,49 @@ __global__ void __launch_bounds__(256) sum_counts_kernel(const int32_t* __restri
     if ((threadIdx.x & 31) == 0 && s != 0) atomicAdd(out, (unsigned long long)s);   // integer: order-independent
 }
 
+// the lookup tables and constants every strip kernel takes (no input or output arrays yet)
+static ConvArgs lookup_args(const hcgrid_ctx* c) {
+    const Region& rg = c->region;
+    ConvArgs a{};
+    a.strips = c->d_strips.as<Strip>();
+    a.wins = c->d_wins.as<RingWin>();
+    a.bin_start = c->d_bins.as<int32_t>();
+    a.rec = c->d_rec.p;
+    a.rg = rg; a.kp = c->kp;
+    a.kmax = c->kmax; a.strip_cells = c->strip_cells;
+    a.raw = c->raw_sums ? 1 : 0;
+    a.small64 = c->f32_series_ok ? 1 : 0;   // R and the longitude half-window <= 0.05 rad, no pole in reach
+    a.qx = (float)(1.0 / rg.sx32);
+    a.qy = (float)(1.0 / rg.sy32);
+    a.sx = rg.sx32;
+    return a;
+}
+
+// pairs the strip kernels (simple, staged, general) put to the distance test: every task of g cells tests each sample
+// of its ring ranges against each of its cells; added to *out
+__global__ void __launch_bounds__(256) strip_pairs_tested_kernel(const ConvArgs a, int g, unsigned long long* out) {
+    const int64_t task = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long pairs = 0;
+    if (task < a.ntasks) {
+        const int s = (int)(task / a.tasks_per_strip);
+        const int ix0 = (int)(task % a.tasks_per_strip) * g;
+        const int ncells = min(g, a.strip_cells - ix0);
+        const int nring = a.strips[s].nring;
+        long long total = 0;
+        for (int k = 0; k < nring; ++k) {
+            int sa, sn, sa2, sn2;
+            ring_segment(a.wins[(size_t)s * a.kmax + k], ix0, ncells, a.rg, a.bin_start, sa, sn, sa2, sn2);
+            total += sn + sn2;
+        }
+        pairs = (unsigned long long)total * (unsigned long long)ncells;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) pairs += __shfl_xor_sync(0xffffffffu, pairs, o);
+    if ((threadIdx.x & 31) == 0 && pairs) atomicAdd(out, pairs);
+}
+
 // The profiling-only figures of hcgrid_stats, after the timed stages: n_hit (sum of the count output) and, for the tile
-// kernel, n_pairs_tested.
+// and the strip kernels, n_pairs_tested.
 int run_profile_stats(hcgrid_ctx* c, int32_t* counts, cudaStream_t st) {
     c->stat_hit = c->stat_pairs = false;
     if (!c->opt_profile) return HCGRID_OK;
@@ -306,6 +351,16 @@ int run_profile_stats(hcgrid_ctx* c, int32_t* counts, cudaStream_t st) {
         const int rc = launch_tile_pairs_tested(c, c->stats.coarsen, c->stats.coarsen_y, c->d_stat.as<unsigned long long>() + 1, st);
         if (rc != HCGRID_OK) return rc;
         c->stat_pairs = true;
+    } else if (c->stats.kernel >= 1 && c->stats.kernel <= 5) {
+        ConvArgs a = lookup_args(c);
+        const int g = c->stats.coarsen > 0 ? c->stats.coarsen : 1;
+        a.tasks_per_strip = (c->strip_cells + g - 1) / g;
+        a.ntasks = (int64_t)a.tasks_per_strip * c->nstrip;
+        if (a.ntasks > 0) {
+            strip_pairs_tested_kernel<<<(unsigned)((a.ntasks + 255) / 256), 256, 0, st>>>(a, g, c->d_stat.as<unsigned long long>() + 1);
+            HCG_CUDA(c, cudaGetLastError());
+        }
+        c->stat_pairs = true;
     }
     return HCGRID_OK;
 }
@@ -313,21 +368,10 @@ int run_profile_stats(hcgrid_ctx* c, int32_t* counts, cudaStream_t st) {
 int run_convolve(hcgrid_ctx* c, int64_t n, const float* values, int nchan, bool has_weights, void* cube,
                  void* wmap, int32_t* counts, cudaStream_t st) {
     const Region& rg = c->region;
-    ConvArgs a{};
-    a.strips = c->d_strips.as<Strip>();
-    a.wins = c->d_wins.as<RingWin>();
-    a.bin_start = c->d_bins.as<int32_t>();
-    a.rec = c->d_rec.p;
+    ConvArgs a = lookup_args(c);
     a.values = values;
     a.cube = cube; a.wmap = wmap; a.counts = counts;
-    a.rg = rg; a.kp = c->kp;
-    a.kmax = c->kmax; a.strip_cells = c->strip_cells;
     a.nchan = nchan;
-    a.raw = c->raw_sums ? 1 : 0;
-    a.small64 = c->f32_series_ok ? 1 : 0;   // R and the longitude half-window <= 0.05 rad, no pole in reach
-    a.qx = (float)(1.0 / rg.sx32);
-    a.qy = (float)(1.0 / rg.sy32);
-    a.sx = rg.sx32;
     const bool f32 = c->precision == HCGRID_F32 && c->f32_series_ok && c->opt_kernel != 2;
     int rc;
     c->stats.coarsen_y = 1;
@@ -384,7 +428,8 @@ int run_convolve(hcgrid_ctx* c, int64_t n, const float* values, int nchan, bool 
         rc = launch_conv_tile(c, n, (float*)cube, (float*)wmap, counts, st);
         c->stats.kernel = 6;
     } else if (f32 && nchan == 1 && c->opt_kernel != 3 && !c->raw_sums) {
-        const bool staged = c->opt_kernel != 1 && c->kmax <= 32;
+        // the staged kernel keeps one sample range per ring: full-circle regions (two ranges on the seam) take the simple one
+        const bool staged = c->opt_kernel != 1 && c->kmax <= 32 && !rg.full_circle;
         int G = c->opt_coarsen;
         if (G == 0) G = c->strip_cells >= 4 ? 2 : 1;
         if (G > c->strip_cells) G = 1;

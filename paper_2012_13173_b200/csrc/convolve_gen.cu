@@ -123,8 +123,10 @@ conv_general(const ConvArgs a) {
         int cnt = 0;
         for (int k = 0; k < st.nring; ++k) {
             const RingWin w = a.wins[(size_t)s * a.kmax + k];
-            int sa, sn;
-            ring_segment(w, ix, 1, a.rg, a.bin_start, sa, sn);
+            int sa, sn, sa2, sn2;
+            ring_segment(w, ix, 1, a.rg, a.bin_start, sa, sn, sa2, sn2);
+            // second range: only where the window crosses the seam of a full-circle region (warp-uniform)
+            for (int seg = 0; seg < 2; ++seg, sa = sa2, sn = sn2)
             for (int base = 0; base < sn; base += 32) {
                 const int i = base + lane;
                 bool hit = false;

@@ -37,12 +37,15 @@ __device__ __forceinline__ float ex2_approx(float x) {
     return y;
 }
 
-// Step (ii)+(iii): sample range of ring-window `w` for the cells [ix0, ix0+g-1].
+// Step (ii)+(iii): sample ranges of ring-window `w` for the cells [ix0, ix0+g-1]: [a, a+n) and, only on a region
+// that spans the whole circle when the pixel window crosses the ring's first pixel, a second range [a2, a2+n2).
+// (Pixel indices of such a window are reduced modulo the ring length nb, so a window on the seam costs its own
+// length, not the whole ring.)
 __device__ __forceinline__ void ring_segment(const RingWin& w, int ix0, int g, const Region& rg,
-                                             const int32_t* __restrict__ bin_start, int& a, int& n) {
-    a = 0; n = 0;
+                                             const int32_t* __restrict__ bin_start, int& a, int& n, int& a2, int& n2) {
+    a = 0; n = 0; a2 = 0; n2 = 0;
     if (w.flags == 0) return;
-    long long jlo, jhi;
+    long long jlo, jhi, klo = 0, khi = -1;
     if (w.flags == 2) {
         jlo = 0; jhi = (w.nb < rg.m ? w.nb : rg.m) - 1;
     } else {
@@ -51,7 +54,16 @@ __device__ __forceinline__ void ring_segment(const RingWin& w, int ix0, int g, c
         jlo = (long long)floor(w.a_lo + (double)ixw * w.step);
         jhi = (long long)floor(w.a_hi + (double)ixe * w.step);
         if (rg.full_circle) {
-            if (jhi - jlo + 1 >= w.nb || jlo < 0 || jhi >= w.nb) { jlo = 0; jhi = w.nb - 1; }
+            const long long len = jhi - jlo + 1;
+            if (len >= w.nb) {
+                jlo = 0; jhi = w.nb - 1;
+            } else {
+                long long j0 = jlo % w.nb;
+                if (j0 < 0) j0 += w.nb;
+                jlo = j0;
+                jhi = j0 + len - 1;
+                if (jhi >= w.nb) { klo = 0; khi = jhi - w.nb; jhi = w.nb - 1; }
+            }
         } else {
             if (jhi < 0 || jlo > rg.m - 1) return;
             if (jlo < 0) jlo = 0;
@@ -61,6 +73,16 @@ __device__ __forceinline__ void ring_segment(const RingWin& w, int ix0, int g, c
     const long long base = (long long)w.ring_rel * rg.m;
     a = __ldg(bin_start + base + jlo);
     n = __ldg(bin_start + base + jhi + 1) - a;
+    if (khi >= klo) {
+        a2 = __ldg(bin_start + base + klo);
+        n2 = __ldg(bin_start + base + khi + 1) - a2;
+    }
+}
+// the same for regions that do not span the circle (never a second range)
+__device__ __forceinline__ void ring_segment(const RingWin& w, int ix0, int g, const Region& rg,
+                                             const int32_t* __restrict__ bin_start, int& a, int& n) {
+    int a2, n2;
+    ring_segment(w, ix0, g, rg, bin_start, a, n, a2, n2);
 }
 
 struct TaskConst {
