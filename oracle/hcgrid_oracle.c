@@ -54,6 +54,36 @@ static double kernel_weight(int ktype, double d, double sigma, double ka, double
     return sinc * exp(-(x / ka) * (x / ka));
 }
 
+/* ktype 2: elliptical Gaussian (reading c17; PAPER.md:186 only names the radially symmetric Gaussian
+ * as the default and follows Winkel et al. 2016b, whose kernel set has a two-dimensional Gaussian).
+ * Polar coordinates of the sample about the cell centre: the great-circle angle d and the bearing beta of the
+ * sample as seen from the cell, measured from north through east (the azimuthal equidistant offsets are
+ * xi = d sin beta towards east, eta = d cos beta towards north).  With phi = beta - PA the angle from the major
+ * axis, u = d cos phi along it and v = d sin phi across it,
+ *     w = exp(-u^2 / (2 smaj^2) - v^2 / (2 smin^2))
+ *       = exp(-( d^2 / (2 smaj^2) + d^2 sin^2(phi) (1 / (2 smin^2) - 1 / (2 smaj^2)) )),
+ * written in the second form so that smin == smaj gives the circular kernel's expression exactly.
+ * The bearing comes from the components of the sample's direction along the cell's east and north unit
+ * vectors, x = cos(lat_s) sin(dlon) and y = cos(lat_c) sin(lat_s) - sin(lat_c) cos(lat_s) cos(dlon), the latter
+ * rewritten as sin(dlat) + 2 sin(lat_c) cos(lat_s) sin^2(dlon / 2) (the same identity that turns the cosine rule
+ * into the haversine form) so that it keeps its accuracy for near pairs; differences are formed in degrees first,
+ * like hcgrid_oracle_distance. */
+static double bearing(double lon_c_deg, double lat_c_deg, double lon_s_deg, double lat_s_deg)
+{
+    const double dlat = (lat_s_deg - lat_c_deg) * DEG2RAD;
+    const double dlon = remainder(lon_s_deg - lon_c_deg, 360.0) * DEG2RAD;
+    const double sb = sin(0.5 * dlon);
+    const double x = cos(lat_s_deg * DEG2RAD) * sin(dlon);
+    const double y = sin(dlat) + 2.0 * sin(lat_c_deg * DEG2RAD) * cos(lat_s_deg * DEG2RAD) * sb * sb;
+    return atan2(x, y);      /* from north (y) through east (x); 0 for a coincident pair */
+}
+
+static double elliptical_weight(double d, double beta, double inv2s2_maj, double inv2s2_min, double pa)
+{
+    const double sphi = sin(beta - pa);
+    return exp(-(d * d * inv2s2_maj + d * d * sphi * sphi * (inv2s2_min - inv2s2_maj)));
+}
+
 static int grid_core(int ktype, double ka, double kb, double sigma_deg, double radius_deg,
                      int64_t ncell, const double* cell_lon, const double* cell_lat,
                      int64_t n, const double* lon, const double* lat,
@@ -70,6 +100,11 @@ static int grid_core(int ktype, double ka, double kb, double sigma_deg, double r
     const double sigma = sigma_deg * DEG2RAD;
     const double R = radius_deg * DEG2RAD;
     const double inv2s2 = 1.0 / (2.0 * sigma * sigma);
+    /* ktype 2: sigma is the standard deviation along the axis at position angle kb (degrees), ka * sigma the one
+     * across it (ka < 1: the axis at the position angle is the major one) */
+    const double sigma_min = sigma * ka;
+    const double inv2s2_min = ktype == 2 ? 1.0 / (2.0 * sigma_min * sigma_min) : inv2s2;
+    const double pa = kb * DEG2RAD;
     /* exact early-out: d >= |dlat| always, so |dlat| > R(1+1e-12) cannot
      * contribute (and cannot be within 1e-9 of R unless R itself is ~1e3) */
     const double dlat_cut_deg = (R * (1.0 + 1e-12) + 1e-9) / DEG2RAD;
@@ -102,7 +137,10 @@ static int grid_core(int ktype, double ka, double kb, double sigma_deg, double r
                 const double d = hcgrid_oracle_distance(clon, clat, lon[s], lat[s]);
                 if (fabs(d - R) < 1e-9) nb++;
                 if (d <= R) {
-                    const double w = ktype == 0 ? exp(-d * d * inv2s2) : kernel_weight(ktype, d, sigma, ka, kb);
+                    const double w = ktype == 0 ? exp(-d * d * inv2s2)
+                                   : ktype == 2 ? elliptical_weight(d, bearing(clon, clat, lon[s], lat[s]), inv2s2,
+                                                                    inv2s2_min, pa)
+                                                : kernel_weight(ktype, d, sigma, ka, kb);
                     const double q = weights ? (double)weights[s] : 1.0;
                     const double qw = q * w;
                     W += (long double)qw;
@@ -120,8 +158,8 @@ static int grid_core(int ktype, double ka, double kb, double sigma_deg, double r
             if (abswmap) abswmap[c] = (double)Wabs;
             if (counts) counts[c] = cnt;
             if (near_boundary) near_boundary[c] = nb;
-            /* Gaussian: W > 0 as soon as one sample contributes.  Signed kernels: W != 0. */
-            const int defined = ktype == 0 ? (W > 0.0L) : (W != 0.0L);
+            /* Gaussians: W > 0 as soon as one sample contributes.  Signed kernels: W != 0. */
+            const int defined = ktype != 1 ? (W > 0.0L) : (W != 0.0L);
             for (int k = 0; k < nchan; ++k) {
                 size_t o = (size_t)c * (size_t)nchan + (size_t)k;
                 if (defined) {
@@ -158,8 +196,9 @@ int hcgrid_oracle_grid_kernel(int ktype, double ka, double kb, double sigma_deg,
                               double* datacube, double* weightmap, int64_t* counts,
                               double* absmap, double* abswmap, int64_t* near_boundary, int nthreads)
 {
-    if (ktype != 0 && ktype != 1) return -1;
+    if (ktype != 0 && ktype != 1 && ktype != 2) return -1;
     if (ktype == 1 && (!(ka > 0.0) || !(kb > 0.0))) return -1;
+    if (ktype == 2 && (!(ka > 0.0) || !(kb == kb))) return -1;
     return grid_core(ktype, ka, kb, sigma_deg, radius_deg, ncell, cell_lon, cell_lat, n, lon, lat, values, nchan,
                      weights, datacube, weightmap, counts, absmap, abswmap, near_boundary, nthreads);
 }

@@ -24,7 +24,10 @@
  *
  * Pins: tests/test_oracle_pins.py (hand case tests/golden/hand_3x3.txt, single
  * sample closed form, constant field, permutation, rotation about the pole
- * axis, closed-form distances, independent vector-formula brute force).
+ * axis, closed-form distances, independent vector-formula brute force; for the
+ * elliptical Gaussian: equality with the circular one at ka = 1, closed forms
+ * along the meridian and the equator, PA + 90 deg swapping the axes, an
+ * independent tangent-vector brute force, constant field).
  */
 #ifndef HCGRID_ORACLE_H
 #define HCGRID_ORACLE_H
@@ -66,6 +69,12 @@ int hcgrid_oracle_grid(double sigma_deg, double radius_deg,
  *   1  tapered sinc: sinc(d / (kb sigma)) * exp(-(d / (ka sigma))^2), sinc(x) = sin(pi x) / (pi x)
  *      (PAPER.md:186 names the sinc as the optimal kernel and finite-length functions as what
  *      is used in practice; the tapered form is that of the work it follows, Winkel et al. 2016b).
+ *   2  elliptical Gaussian exp(-u^2 / (2 s1^2) - v^2 / (2 s2^2)) (reading c17): s1 = sigma_deg is the
+ *      standard deviation along the axis at position angle kb (degrees, from north through east), s2 = ka * s1
+ *      (ka > 0; ka < 1 makes the axis at the position angle the major one) the one across it;
+ *      (u, v) = d (cos(beta - PA), sin(beta - PA)) with d the great-circle angle and beta the bearing of the
+ *      sample from the cell centre; the support stays the circle d <= R (reading c4).  ka = 1 gives ktype 0 bit
+ *      for bit.
  * Signed weights change two outputs: datacube = S / W wherever W != 0 (NaN otherwise), and
  * absmap = sum |q w| |v| / |W|.  abswmap[ncell] (may be NULL) = sum |q w|, the scale against
  * which W itself is to be compared (W can cancel to ~0).  Returns 0, or -1 on invalid arguments. */

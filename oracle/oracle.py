@@ -73,7 +73,7 @@ def _ptr(a):
     return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
 
 
-GAUSS, TAPERED_SINC = 0, 1
+GAUSS, TAPERED_SINC, ELLIPTICAL_GAUSS = 0, 1, 2
 
 
 def _vmax(values) -> float:

@@ -316,3 +316,141 @@ def test_tapered_sinc_constant_field_and_negative_lobes(oracle):
         oracle.grid(0.1, 0.3, [0.0], [0.0], [0.0], [0.0], [1.0], kernel=(1, 2.52, 0.0))
     with pytest.raises(ValueError):
         oracle.grid(0.1, 0.3, [0.0], [0.0], [0.0], [0.0], [1.0], kernel=(7, 1.0, 1.0))
+
+
+# ---------------------------------------------------------------- elliptical Gaussian kernel (S:8f NEXT-3, reading c17)
+def _ell(oracle, s1, ratio, pa, clon, clat, lon, lat, val=None, wts=None, radius=None):
+    val = np.ones(np.size(lon), np.float32) if val is None else val
+    return oracle.grid(s1, radius or 5 * s1 * max(1.0, ratio), clon, clat, lon, lat, val, wts,
+                       kernel=(oracle.ELLIPTICAL_GAUSS, ratio, pa))
+
+
+def test_elliptical_equals_the_circular_gaussian_at_ratio_one(oracle):
+    """s2 = s1: the exponent's second term is exactly zero, whatever the position angle -- bit for bit the routine
+    pinned above.  Catches: any change to the distance, the support test or the accumulation on the ktype-2 path."""
+    rng = np.random.default_rng(21)
+    n = 500
+    lon = 359.8 + rng.uniform(-0.5, 0.5, n)
+    lat = 70.0 + rng.uniform(-0.5, 0.5, n)
+    val = rng.normal(size=(n, 2)).astype(np.float32)
+    wts = rng.uniform(0.5, 2.0, n).astype(np.float32)
+    clon, clat = np.meshgrid(359.8 + np.linspace(-0.4, 0.4, 6), 70.0 + np.linspace(-0.4, 0.4, 5))
+    g = oracle.grid(0.06, 0.21, clon, clat, lon, lat, val, wts)
+    for pa in (0.0, 33.0, -120.0):
+        e = oracle.grid(0.06, 0.21, clon, clat, lon, lat, val, wts, kernel=(oracle.ELLIPTICAL_GAUSS, 1.0, pa))
+        assert np.array_equal(e.weightmap, g.weightmap) and np.array_equal(e.counts, g.counts)
+        assert np.array_equal(e.datacube, g.datacube, equal_nan=True)
+
+
+def test_elliptical_closed_forms_along_the_axes(oracle):
+    """One sample due north / south of the cell (same meridian: d = |dlat|, bearing 0 / 180 deg) and one due east on
+    the equator (d = dlon, bearing 90 deg).  PA = 0 puts axis 1 on the meridian, PA = 90 on the east-west line, PA = 45
+    halves sin^2.  Catches: s1 and s2 swapped, PA measured from east, degrees taken as radians, a dropped 1/2."""
+    s1, ratio = 0.1, 0.4
+    s2 = s1 * ratio
+    d = 0.07
+    g1, g2 = math.exp(-d * d / (2 * s1 * s1)), math.exp(-d * d / (2 * s2 * s2))
+    g45 = math.exp(-d * d / 4 * (1 / s1 ** 2 + 1 / s2 ** 2))
+    for (clon, clat, slon, slat) in [(40.0, 10.0, 40.0, 10.0 + d), (40.0, 10.0, 40.0, 10.0 - d),
+                                     (200.0, -35.0, 200.0, -35.0 + d), (12.0, 0.0, 12.0 + d, 0.0),
+                                     (359.99, 0.0, 359.99 + d - 360.0, 0.0), (12.0, 0.0, 12.0 - d, 0.0)]:
+        on_meridian = clon == slon
+        for pa, want in [(0.0, g1 if on_meridian else g2), (90.0, g2 if on_meridian else g1), (180.0, g1 if on_meridian else g2),
+                         (-90.0, g2 if on_meridian else g1), (45.0, g45), (135.0, g45)]:
+            w = _ell(oracle, s1, ratio, pa, [clon], [clat], [slon], [slat], radius=0.2).weightmap[0]
+            assert w == pytest.approx(want, rel=2e-12), (clon, clat, slon, slat, pa)
+    # coincident pair: weight 1 whatever the angle (the bearing of a zero offset is irrelevant)
+    assert _ell(oracle, s1, ratio, 77.0, [5.0], [5.0], [5.0], [5.0], radius=0.2).weightmap[0] == 1.0
+
+
+def test_elliptical_position_angle_runs_from_north_through_east(oracle):
+    """A sample to the north-east of a cell on the equator, placed so that its bearing is exactly 45 deg
+    (tan lat_s = sin dlon): PA = +45 puts it on axis 1, PA = -45 on axis 2.  Catches a mirrored position angle
+    (north through west) and a bearing built with the arguments of atan2 exchanged."""
+    s1, ratio = 0.1, 0.5
+    dlon = 0.05
+    slat = math.degrees(math.atan(math.sin(math.radians(dlon))))
+    d = oracle.distance(30.0, 0.0, 30.0 + dlon, slat)
+    on1 = math.exp(-d * d / (2 * math.radians(s1) ** 2))
+    on2 = math.exp(-d * d / (2 * math.radians(s1 * ratio) ** 2))
+    assert _ell(oracle, s1, ratio, 45.0, [30.0], [0.0], [30.0 + dlon], [slat]).weightmap[0] == pytest.approx(on1, rel=1e-11)
+    assert _ell(oracle, s1, ratio, -45.0, [30.0], [0.0], [30.0 + dlon], [slat]).weightmap[0] == pytest.approx(on2, rel=1e-11)
+    # the mirror image (north-west) swaps the two
+    assert _ell(oracle, s1, ratio, 45.0, [30.0], [0.0], [30.0 - dlon], [slat]).weightmap[0] == pytest.approx(on2, rel=1e-11)
+
+
+def test_elliptical_quarter_turn_swaps_the_axes_and_half_turn_changes_nothing(oracle):
+    """(s1, s2, PA) and (s2, s1, PA + 90) describe the same ellipse; PA + 180 is the same axis."""
+    rng = np.random.default_rng(22)
+    n = 600
+    lon = 120.0 + rng.uniform(-0.6, 0.6, n)
+    lat = -48.0 + rng.uniform(-0.4, 0.4, n)
+    val = rng.normal(size=(n, 2)).astype(np.float32)
+    clon, clat = np.meshgrid(120.0 + np.linspace(-0.4, 0.4, 6), -48.0 + np.linspace(-0.3, 0.3, 5))
+    s1, ratio, pa, radius = 0.09, 0.45, 27.0, 0.3
+    a = oracle.grid(s1, radius, clon, clat, lon, lat, val, kernel=(oracle.ELLIPTICAL_GAUSS, ratio, pa))
+    b = oracle.grid(s1 * ratio, radius, clon, clat, lon, lat, val, kernel=(oracle.ELLIPTICAL_GAUSS, 1.0 / ratio, pa + 90.0))
+    c = oracle.grid(s1, radius, clon, clat, lon, lat, val, kernel=(oracle.ELLIPTICAL_GAUSS, ratio, pa + 180.0))
+    assert a.counts.sum() > 0 and np.array_equal(a.counts, b.counts)
+    assert np.allclose(a.weightmap, b.weightmap, rtol=1e-11) and np.allclose(a.weightmap, c.weightmap, rtol=1e-11)
+    assert np.allclose(a.datacube, b.datacube, rtol=1e-10, atol=1e-12, equal_nan=True)
+    assert np.allclose(a.datacube, c.datacube, rtol=1e-10, atol=1e-12, equal_nan=True)
+    # and it is not the circular kernel
+    g = oracle.grid(s1, radius, clon, clat, lon, lat, val)
+    assert np.abs(a.weightmap - g.weightmap).max() > 1e-3 * g.weightmap.max()
+
+
+@pytest.mark.parametrize("lon_c,lat_c,pa", [(0.0, 0.0, 30.0), (359.9, 62.0, -71.0), (181.0, -88.9, 100.0), (45.0, 89.5, 10.0)])
+def test_elliptical_brute_force_with_tangent_vectors(oracle, lon_c, lat_c, pa):
+    """Independent brute force in numpy: unit vectors, the cell's east / north tangent vectors, d from
+    atan2(|c x s|, c . s), offsets along and across the axis by rotating (east, north) components -- the first form of
+    the exponent, none of the oracle's haversine / bearing identities.  Includes polar caps and the lon = 0 seam."""
+    rng = np.random.default_rng(23)
+    n = 300
+    s1, ratio, radius = 0.2, 0.35, 0.7
+    lat = np.clip(lat_c + rng.uniform(-0.8, 0.8, n), -90.0, 90.0)
+    lon = np.mod(lon_c + rng.uniform(-0.8, 0.8, n) / max(math.cos(math.radians(lat_c)), 0.02), 360.0)
+    val = rng.normal(size=(n, 1)).astype(np.float32)
+    wts = rng.uniform(0.5, 1.5, n).astype(np.float32)
+    clat = np.clip(lat_c + np.array([-0.3, 0.0, 0.25, 0.4]), -89.99, 89.99)
+    clon = np.mod(lon_c + np.array([0.2, 0.0, -0.3, 0.1]), 360.0)
+    res = oracle.grid(s1, radius, clon, clat, lon, lat, val, wts, kernel=(oracle.ELLIPTICAL_GAUSS, ratio, pa))
+
+    def unit(lo, la):
+        lo, la = np.radians(lo), np.radians(la)
+        return np.stack([np.cos(la) * np.cos(lo), np.cos(la) * np.sin(lo), np.sin(la)], -1)
+    s = unit(lon, lat)
+    S1, S2, R, PA = math.radians(s1), math.radians(s1 * ratio), math.radians(radius), math.radians(pa)
+    for i in range(clon.size):
+        c = unit(clon[i], clat[i])
+        lo, la = math.radians(clon[i]), math.radians(clat[i])
+        east = np.array([-math.sin(lo), math.cos(lo), 0.0])
+        north = np.array([-math.sin(la) * math.cos(lo), -math.sin(la) * math.sin(lo), math.cos(la)])
+        d = np.arctan2(np.linalg.norm(np.cross(c, s), axis=1), s @ c)
+        x, y = s @ east, s @ north
+        r = np.hypot(x, y)
+        xi, eta = d * x / r, d * y / r                       # azimuthal equidistant offsets (east, north)
+        u = eta * math.cos(PA) + xi * math.sin(PA)            # along the axis at PA (from north through east)
+        v = xi * math.cos(PA) - eta * math.sin(PA)            # across it
+        hit = d <= R
+        assert np.abs(d - R).min() > 1e-7                     # no pair near the boundary in this draw
+        w = np.exp(-u * u / (2 * S1 * S1) - v * v / (2 * S2 * S2)) * wts * hit
+        assert res.counts[i] == hit.sum() and hit.sum() > 0
+        assert res.weightmap[i] == pytest.approx(w.sum(), rel=1e-9)
+        assert res.datacube[i, 0] == pytest.approx((w * val[:, 0]).sum() / w.sum(), rel=1e-8, abs=1e-11)
+
+
+def test_elliptical_constant_field_and_errors(oracle):
+    rng = np.random.default_rng(24)
+    n = 2000
+    lon = 10.0 + rng.uniform(-1, 1, n)
+    lat = 50.0 + rng.uniform(-1, 1, n)
+    clon, clat = np.meshgrid(10.0 + np.linspace(-0.8, 0.8, 9), 50.0 + np.linspace(-0.8, 0.8, 9))
+    res = oracle.grid(0.1, 0.3, clon, clat, lon, lat, np.full(n, -1.75, np.float32),
+                      kernel=(oracle.ELLIPTICAL_GAUSS, 0.5, 60.0))
+    assert np.all(res.counts > 0) and np.all(res.weightmap > 0)
+    assert np.allclose(res.datacube[:, 0], -1.75, rtol=1e-12)
+    with pytest.raises(ValueError):
+        oracle.grid(0.1, 0.3, [0.0], [0.0], [0.0], [0.0], [1.0], kernel=(2, 0.0, 10.0))
+    with pytest.raises(ValueError):
+        oracle.grid(0.1, 0.3, [0.0], [0.0], [0.0], [0.0], [1.0], kernel=(2, 0.5, float("nan")))
