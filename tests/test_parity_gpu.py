@@ -357,11 +357,32 @@ def sampled_cells(ncell, nx, k, seed):
     return np.unique(np.concatenate([border, inner])).astype(np.int64)
 
 
-@pytest.mark.parametrize("cfg,k", [(2, 600), (3, 300), (4, 150), (5, 120)])
+def golden_reference(w, cfg):
+    """The oracle's results on the declared stratified subset (borders 8 cells deep + 64 seeded 32 x 32 interior
+    blocks) of a full-size config, written once by tests/make_golden.py -- which calls only oracle/ --
+    and keyed by a hash of the kernel, the target and the input arrays."""
+    from golden_subset import golden_path, subset_cells, workload_key
+    from oracle.oracle import OracleResult
+    z = np.load(golden_path(cfg))
+    assert str(z["key"]) == workload_key(w), "tests/golden is stale: rerun tests/make_golden.py"
+    cells = subset_cells(w.target.nx, w.target.ny, cfg)
+    assert np.array_equal(cells, z["cells"])
+    ref = OracleResult(z["datacube"], z["weightmap"], z["counts"].astype(np.int64), z["absmap"],
+                       z["near_boundary"].astype(np.int64), 0, None, float(z["vmax"]))
+    return cells, ref
+
+
+@pytest.mark.parametrize("cfg,k", [(2, 600), (3, 0), (4, 150), (5, 0)])
 def test_full_size_sampled_cells(oracle, cfg, k):
+    """Full-size configs in the launch configuration bench.py times.  Configs 3 and 5: ~1e5 and ~8e4 cells (the
+    stratified subset, oracle results from tests/golden); configs 2 and 4: sampled cells computed live."""
     w = workloads.make(cfg, 1.0)
-    cells = sampled_cells(w.target.ncell, w.target.nx, k, cfg)
-    ref = run_oracle(oracle, w, cells)
+    if cfg in (3, 5):
+        cells, ref = golden_reference(w, cfg)
+        assert cells.size > 60000
+    else:
+        cells = sampled_cells(w.target.ncell, w.target.nx, k, cfg)
+        ref = run_oracle(oracle, w, cells)
     cube, wmap, cnt, st = run_gpu(w, "f32")          # default options, with the count output
     r = compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F32, qmax(w), cells=cells)
     assert r["n_hit"] > 0
@@ -374,10 +395,25 @@ def test_full_size_sampled_cells(oracle, cfg, k):
     assert np.array_equal(wmap > 0, cnt > 0)
     assert np.array_equal(np.isfinite(cube[:, 0]), cnt > 0)
     assert cnt.min() >= 0 and cnt.max() <= w.n
-    if cfg == 3:
-        # fp64 mode at the target config, same sampled cells
+    if cfg in (3, 5):
+        # fp64 mode at full size, same cells
         cube, wmap, cnt, _ = run_gpu(w, "f64")
-        compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F64, cells=cells)
+        compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F64, qmax(w), cells=cells)
+
+
+@pytest.mark.parametrize("precision,tol", [("f32", TOL_F32), ("f64", TOL_F64)])
+def test_support_radius_of_five_sigma(oracle, precision, tol):
+    """The upper end of the paper's sphere_radius range ("3 sigma_kernel - 5 sigma_kernel"): config 1
+    with R = 5 sigma exactly (weights down to exp(-12.5) = 3.7e-6 at the edge), both precisions, with and
+    without per-sample weights."""
+    w = workloads.make(1, 1.0)
+    w.radius_deg = 5.0 * w.sigma_deg
+    for wts in (None, np.random.default_rng(55).uniform(0.5, 1.5, w.n).astype(np.float32)):
+        w.weights = wts
+        ref = run_oracle(oracle, w)
+        cube, wmap, cnt, st = run_gpu(w, precision)
+        r = compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, tol, qmax(w))
+        assert r["n_hit"] > 2.5 * 1.27e6                  # (5 / 3)^2 times config 1's pairs
 
 
 # ------------------------------------------------------------ randomised plate-carree targets
@@ -388,7 +424,7 @@ def _random_car_case(seed):
     lat_c = float(rng.uniform(-84.0, 84.0))
     lon_c = float(rng.choice([0.0, 359.7, 0.2, rng.uniform(0.0, 360.0)]))
     sigma = float(rng.uniform(0.6, 3.0)) / 60.0
-    radius = sigma * float(rng.uniform(2.5, 4.0))
+    radius = sigma * float(rng.uniform(2.5, 5.0))               # the paper's range of sphere_radius: 3 - 5 sigma
     cell = sigma * float(rng.uniform(0.5, 1.2))
     nx, ny = int(rng.integers(5, 42)), int(rng.integers(5, 34))
     sx, sy = (1.0 if rng.random() < 0.5 else -1.0), (1.0 if rng.random() < 0.5 else -1.0)
@@ -475,7 +511,7 @@ def test_random_polar_and_wide_kernels(oracle, seed):
     else:
         lat_c = float(rng.uniform(-70.0, 70.0))
         sigma = float(rng.uniform(5.0, 40.0)) / 60.0          # up to 0.67 deg
-    radius = sigma * float(rng.uniform(2.5, 3.5))
+    radius = sigma * float(rng.uniform(2.5, 5.0))               # 3 - 5 sigma and a little below
     cell = sigma * float(rng.uniform(0.6, 1.2))
     nx, ny = int(rng.integers(4, 30)), int(rng.integers(3, 12))
     ny = max(1, min(ny, int((89.95 - abs(lat_c)) / (0.5 * cell)))) if polar else ny
@@ -506,6 +542,44 @@ def test_random_polar_and_wide_kernels(oracle, seed):
     compare(cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy(), ref, sigma, radius, TOL_F32,
             1.5 if wts is not None else 1.0)
     g.close()
+
+
+@pytest.mark.parametrize("kernel,precision", [(1, "f32"), (3, "f32"), (0, "f64")])
+def test_all_sky_target_starting_at_minus_180(oracle, kernel, precision):
+    """A target that spans the whole circle and starts at lon = -180: the region is a full-circle region and every
+    pixel window west of lon = 0 has negative pixel indices.  Windows are reduced modulo the ring length (two sample
+    ranges where one crosses the ring's first pixel) instead of widening to the whole ring, so the number of pairs
+    put to the distance test stays a small multiple of the hits on both halves of the sky."""
+    from paper_2012_13173_b200 import binding
+    rng = np.random.default_rng([13173, 808])
+    n = 150000
+    lon = rng.uniform(0.0, 360.0, n)
+    lat = np.rad2deg(np.arcsin(rng.uniform(np.sin(np.deg2rad(-62.0)), np.sin(np.deg2rad(62.0)), n)))
+    val = rng.standard_normal((n, 1)).astype(np.float32)
+    sigma, radius = 0.4, 1.2
+    tgt = workloads.CarTarget(360, 61, -180.0, -60.0, 1.0, 2.0)
+    cl, cb = tgt.cell_centers()
+    ref = oracle.grid(sigma, radius, cl, cb, lon, lat, val, None)
+    pairs = {}
+    for lon0 in (-180.0, 0.0, 97.0):                # the same 360 cells per row, listed from three starting points
+        g = binding.HCGrid(sigma, radius, 256, precision=precision)
+        g.set_option(binding.OPT_PROFILE, 1)
+        if kernel:
+            g.set_option(binding.OPT_KERNEL, kernel)
+        g.set_target_car(tgt.nx, tgt.ny, lon0, tgt.lat0, tgt.dlon, tgt.dlat)
+        cube, wmap, cnt = g.grid(_dev(lon), _dev(lat), _dev(val))
+        torch.cuda.synchronize()
+        st = g.stats()
+        g.close()
+        assert st["kernel"] == (kernel if kernel else 5)
+        assert st["n_hit"] == int(cnt.sum().item()) == int(ref.counts.sum())
+        assert st["n_pairs_tested"] >= st["n_hit"]
+        pairs[lon0] = st["n_pairs_tested"]
+        assert pairs[lon0] < 8 * st["n_hit"], (lon0, st)     # a whole-ring scan would test ~100 x the hits
+        if lon0 == -180.0:
+            compare(cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy(), ref, sigma, radius,
+                    TOL_F32 if precision == "f32" else TOL_F64)
+    assert max(pairs.values()) < 1.05 * min(pairs.values()), pairs
 
 
 def test_large_sparse_target(oracle):
