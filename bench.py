@@ -43,6 +43,7 @@ UNIT = "cell-channels/s"
 NCU_TRAFFIC = {
     (3, 6): (191985408 + 12509952, "profiles/r01e_conv1_tile_ncu_full.md"),
     (4, 7): (3714980000 + 98979072, "profiles/r01c_conv_mc_ncu_full.md"),
+    (4, 8): (1368034000 + 81781760, "profiles/r02_conv_mc_tc_ncu_full.md"),
 }
 WORKLOAD_NAMES = {1: "config1_tiny_20k", 2: "config2_drift_scan_1.25M", 3: "config3_dense_10M",
                   4: "config4_spectral_cube_1M_x256", 5: "config5_polar_20M"}
@@ -195,7 +196,15 @@ def run_product(args):
         w.weights = None if w.weights is None else w.weights[m]
     t = w.target
     g = binding.HCGrid(w.sigma_deg, w.radius_deg, w.nside, precision="f32", device=local)
-    g.set_target_car(t.nx, t.ny, t.lon0, t.lat0, t.dlon, t.dlat)
+    if args.kernel_function == "sinc":                 # variants, not the headline: DESIGN.md "Kernel functions"
+        g.set_kernel(binding.KERNEL_TAPERED_SINC, 2.52, 1.55)
+    elif args.kernel_function == "elliptical":
+        g.set_kernel(binding.KERNEL_ELLIPTICAL_GAUSS, 0.5, 30.0)
+    if args.explicit_cells:                            # the same cells handed over one by one (hcgrid_set_target_cells)
+        cl, cb = t.cell_centers()
+        g.set_target_cells(torch.from_numpy(cl).to(dev), torch.from_numpy(cb).to(dev))
+    else:
+        g.set_target_car(t.nx, t.ny, t.lon0, t.lat0, t.dlon, t.dlat)
     lon, lat = torch.from_numpy(w.lon).to(dev), torch.from_numpy(w.lat).to(dev)
     val = torch.from_numpy(w.values).to(dev)
     wts = None if w.weights is None else torch.from_numpy(w.weights).to(dev)
@@ -318,10 +327,17 @@ def run_product(args):
         "frac_of_measured_issue_rate": (mdl["fp32_inst"] / t_conv) / p_fp32_meas if p_fp32_meas > 0 else None,
         "hbm_gbs_achieved_unique_bytes": mdl["bytes_unique"] / t_conv / 1e9,
     })
+    # the contract exactly as SURVEY.md 8d wrote it: F_a = 6 + nchan per accepted pair (the count increment always
+    # charged) against the kernel that does write the count output
+    if mdl["bound"] == "alu":
+        t_cnt = float(np.median(us_conv_counts)) * 1e-6
+        inst_s = cand["n_cand"] * roofline.F_D + n_hit * (6 + nchan + (1 if w.weights is not None else 0))
+        rl["survey_contract"] = {"f_a": 6 + nchan, "fp32_inst": inst_s, "kernel_us_with_count_output": t_cnt * 1e6,
+                                 "frac": inst_s / t_cnt / roofline.P_FP32_NOMINAL}
 
     # ---- oracle on this box's host cores, bounded sample
     cpu = None
-    if world == 1 and not args.no_cpu_baseline:
+    if world == 1 and not args.no_cpu_baseline and args.kernel_function == "gauss":
         k = cpu_cells_per_step(w, args.cpu_seconds)
         cells = evenly_spaced_cells(ncell, k)
         ref, tcpu = oracle_sample(w, cells)
@@ -350,7 +366,9 @@ def run_product(args):
                    "coarsen": st["coarsen"], "coarsen_y": st["coarsen_y"], "subpix_bits": st["subpix_bits"],
                    "preorder": {1: "radix sort", 2: "counting sort"}.get(st["preorder"], "?"),
                    "e2e_path": "hcgrid_grid_host, pinned buffers; inputs of 64 MB or more are copied in 4 pieces and gridded as they arrive", "per_rank": "one independent problem" if units_total is None else "a band of target rows + its samples (rank 0's figures in roofline / stages)",
-                   "outputs": "datacube + weight map (count output off in the timed calls)"},
+                   "outputs": "datacube + weight map (count output off in the timed calls)",
+                   "kernel_function": args.kernel_function,
+                   "target": "per-cell lon/lat (hcgrid_set_target_cells)" if args.explicit_cells else "CAR parameters"},
         "kernel_evals_per_s": n_hit * world * args.steps / (ms_total * 1e-3),
         "conv_kernel": {"us": t_conv * 1e6, "cell_channels_per_s": ncell * nchan / t_conv,
                         "kernel_evals_per_s": n_hit / t_conv,
@@ -412,6 +430,11 @@ def main():
     ap.add_argument("--cand-rows", type=int, default=None, help="count N_cand on this many rows and scale")
     ap.add_argument("--shard", default="replicas", choices=["replicas", "rows"],
                     help="N > 1: independent replicas (weak scaling, default) or one problem cut into row bands (strong)")
+    ap.add_argument("--kernel-function", default="gauss", choices=["gauss", "sinc", "elliptical"],
+                    help="kernel function of Eq. 1: the paper's Gaussian (default), the tapered sinc (a 2.52, b 1.55) or "
+                         "the elliptical Gaussian (ratio 0.5, position angle 30 deg)")
+    ap.add_argument("--explicit-cells", action="store_true",
+                    help="hand the target over as per-cell lon/lat (hcgrid_set_target_cells) instead of CAR parameters")
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per launch of the convolution kernel from the committed ncu capture")
     args = ap.parse_args()

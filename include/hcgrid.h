@@ -116,11 +116,17 @@ int hcgrid_set_option(hcgrid_ctx* ctx, int option, int64_t value);
  *                               b = 1.55; the caller's choice here).  Weights can
  *                               be negative: the datacube is S / W wherever W != 0 (NaN otherwise) and the
  *                               weight map may cancel towards zero.
+ *   HCGRID_KERNEL_ELLIPTICAL_GAUSS  exp(-u^2 / (2 s1^2) - v^2 / (2 s2^2)) (reading c21; PAPER.md:186
+ *                               names only the radially symmetric Gaussian): s1 = the context's sigma along the
+ *                               axis at position angle b (degrees, from north through east), s2 = a * s1 across
+ *                               it (a > 0; a < 1: the axis at the position angle is the major one).  (u, v) =
+ *                               d (cos(beta - b), sin(beta - b)), d the great-circle angle and beta the bearing
+ *                               of the sample seen from the cell centre.  The support stays the circle d <= R.
  * Takes effect at the next hcgrid_grid / hcgrid_accumulate; not allowed while an accumulation is open.
  * Gaussian runs on every convolution kernel; other functions on the general kernels only
  * (any target, any channel count, both precisions).  Returns HCGRID_ERR_INVALID_ARG for an
- * unknown type or non-positive a, b. */
-enum { HCGRID_KERNEL_GAUSS = 0, HCGRID_KERNEL_TAPERED_SINC = 1 };
+ * unknown type, non-positive a (b for the sinc) or non-finite a, b. */
+enum { HCGRID_KERNEL_GAUSS = 0, HCGRID_KERNEL_TAPERED_SINC = 1, HCGRID_KERNEL_ELLIPTICAL_GAUSS = 2 };
 int hcgrid_set_kernel(hcgrid_ctx* ctx, int32_t kernel_type, double a, double b);
 
 /* Target = plate-carree grid: cell (ix, iy) centre = (lon0 + ix*dlon, lat0 + iy*dlat),

@@ -31,7 +31,7 @@ EXPORTS = [
     "hcgrid_measure_peaks", "hcgrid_accumulate", "hcgrid_finalize", "hcgrid_accumulated_batches",
     "hcgrid_set_kernel",
 ]
-KERNEL_GAUSS, KERNEL_TAPERED_SINC = 0, 1          # hcgrid_set_kernel types
+KERNEL_GAUSS, KERNEL_TAPERED_SINC, KERNEL_ELLIPTICAL_GAUSS = 0, 1, 2          # hcgrid_set_kernel types
 
 
 class HCGridError(RuntimeError):
@@ -193,7 +193,8 @@ class HCGrid:
         self._check(self._lib.hcgrid_set_option(self._ctx, option, int(value)))
 
     def set_kernel(self, kernel_type: int, a: float = 0.0, b: float = 0.0):
-        """hcgrid_set_kernel: KERNEL_GAUSS (default) or KERNEL_TAPERED_SINC with its a, b."""
+        """hcgrid_set_kernel: KERNEL_GAUSS (default), KERNEL_TAPERED_SINC with its a, b, or KERNEL_ELLIPTICAL_GAUSS with
+        a = sigma across / sigma along the axis and b = position angle of the axis (degrees, north through east)."""
         self._check(self._lib.hcgrid_set_kernel(self._ctx, int(kernel_type), float(a), float(b)))
 
     def set_target_car(self, nx: int, ny: int, lon0_deg: float, lat0_deg: float, dlon_deg: float,

@@ -149,6 +149,20 @@ int hcgrid_set_kernel(hcgrid_ctx* c, int32_t kernel_type, double a, double b) {
         kp.ktype = HCGRID_KERNEL_GAUSS;
         return HCGRID_OK;
     }
+    if (kernel_type == HCGRID_KERNEL_ELLIPTICAL_GAUSS) {
+        // a = sigma_2 / sigma_1 (across / along the axis), b = position angle of the axis in degrees
+        if (!(a > 0.0) || !std::isfinite(a) || !std::isfinite(b))
+            return fail(c, HCGRID_ERR_INVALID_ARG, "elliptical Gaussian needs a finite axis ratio a > 0 and a finite position angle b");
+        const double s2 = kp.sigma * a;
+        kp.ktype = HCGRID_KERNEL_ELLIPTICAL_GAUSS;
+        kp.ell_k = 1.0 / (2.0 * s2 * s2) - kp.inv2s2;
+        kp.ell_cp = std::cos(b * kDeg2Rad);
+        kp.ell_sp = std::sin(b * kDeg2Rad);
+        kp.ek2 = (float)(-kp.ell_k * 1.4426950408889634);
+        kp.ecp = (float)kp.ell_cp;
+        kp.esp = (float)kp.ell_sp;
+        return HCGRID_OK;
+    }
     if (kernel_type != HCGRID_KERNEL_TAPERED_SINC) return fail(c, HCGRID_ERR_INVALID_ARG, "unknown kernel type %d", (int)kernel_type);
     if (!(a > 0.0) || !(b > 0.0) || !std::isfinite(a) || !std::isfinite(b))
         return fail(c, HCGRID_ERR_INVALID_ARG, "tapered sinc needs a > 0 and b > 0");

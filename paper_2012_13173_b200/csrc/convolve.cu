@@ -305,7 +305,7 @@ static ConvArgs lookup_args(const hcgrid_ctx* c) {
     a.rg = rg; a.kp = c->kp;
     a.kmax = c->kmax; a.strip_cells = c->strip_cells;
     a.raw = c->raw_sums ? 1 : 0;
-    a.small64 = c->f32_series_ok ? 1 : 0;   // R and the longitude half-window <= 0.05 rad, no pole in reach
+    a.small64 = c->small_series_ok ? 1 : 0;   // R and the longitude half-window <= 0.05 rad, no pole in reach
     a.qx = (float)(1.0 / rg.sx32);
     a.qy = (float)(1.0 / rg.sy32);
     a.sx = rg.sx32;

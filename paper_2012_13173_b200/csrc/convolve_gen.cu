@@ -44,10 +44,20 @@ __device__ __forceinline__ float tapered_sinc32(float e2, const KernelParams& kp
     return sinc * ex2_approx(-t * kp.tg2);
 }
 
+// Elliptical Gaussian (reading c21).  x, y: components of the sample's direction along the cell's east
+// and north unit vectors (x = cos(lat_s) sin(dlon), y = sin(dlat) + 2 sin(lat_c) cos(lat_s) sin^2(dlon / 2));
+// sin(beta - PA) = (x cos PA - y sin PA) / hypot(x, y), beta the bearing from north through east.
+__device__ __forceinline__ double elliptical64(double d2, double x, double y, const KernelParams& kp) {
+    const double r2 = x * x + y * y;
+    const double t = x * kp.ell_cp - y * kp.ell_sp;
+    const double s2phi = r2 > 0.0 ? t * t / r2 : 0.0;
+    return exp(-(d2 * kp.inv2s2 + d2 * s2phi * kp.ell_k));
+}
+
 // fp64 pair: returns hit; w = q-less kernel weight.  The definition with no shortcut:
 // differences formed in degrees first, haversine, d = 2 asin(sqrt(hav)), w = exp(-d^2/(2 sigma^2)).
 template <int KFN>
-__device__ __forceinline__ bool pair64(const Rec64& r, double clon_deg, double clat_deg, double ccos,
+__device__ __forceinline__ bool pair64(const Rec64& r, double clon_deg, double clat_deg, double ccos, double csin,
                                        const KernelParams& kp, double& w) {
     const double dlat = (r.lat_deg - clat_deg) * kDeg2Rad;
     const double dlon = remainder(r.lon_deg - clon_deg, 360.0) * kDeg2Rad;
@@ -55,7 +65,10 @@ __device__ __forceinline__ bool pair64(const Rec64& r, double clon_deg, double c
     double hav = sa * sa + ccos * r.coslat * sb * sb;
     if (hav > 1.0) hav = 1.0;
     const double d = 2.0 * asin(sqrt(hav));
-    w = KFN == 0 ? exp(-d * d * kp.inv2s2) : tapered_sinc64(d * d, kp);
+    if (KFN == 2)
+        w = elliptical64(d * d, r.coslat * sin(dlon), sin(dlat) + 2.0 * csin * r.coslat * sb * sb, kp);
+    else
+        w = KFN == 0 ? exp(-d * d * kp.inv2s2) : tapered_sinc64(d * d, kp);
     return d <= kp.radius;
 }
 
@@ -72,17 +85,49 @@ __device__ __forceinline__ double sin2_small(double y) {
 // result agrees with pair64 far inside the 1e-12 tier while costing a third of its fp64 instructions.
 // d <= R is tested as hav <= sin^2(R/2) (the same statement, asin and sqrt being monotone).
 template <int KFN>
-__device__ __forceinline__ bool pair64_small(const Rec64& r, double clon_deg, double clat_deg, double ccos,
+__device__ __forceinline__ bool pair64_small(const Rec64& r, double clon_deg, double clat_deg, double ccos, double csin,
                                              const KernelParams& kp, double& w) {
     const double dlat = (r.lat_deg - clat_deg) * kDeg2Rad;
     const double dlon = remainder(r.lon_deg - clon_deg, 360.0) * kDeg2Rad;
-    const double h = sin2_small(0.5 * dlat) + ccos * r.coslat * sin2_small(0.5 * dlon);
+    const double sb2 = sin2_small(0.5 * dlon);
+    const double h = sin2_small(0.5 * dlat) + ccos * r.coslat * sb2;
     const double d2 = 4.0 * h * fma(h, fma(h, fma(h, fma(h, 128.0 / 1575.0, 4.0 / 35.0), 8.0 / 45.0), 1.0 / 3.0), 1.0);
-    w = KFN == 0 ? exp(-d2 * kp.inv2s2) : tapered_sinc64(d2, kp);
+    if (KFN == 2)
+        w = elliptical64(d2, r.coslat * sin(dlon), sin(dlat) + 2.0 * csin * r.coslat * sb2, kp);
+    else
+        w = KFN == 0 ? exp(-d2 * kp.inv2s2) : tapered_sinc64(d2, kp);
     return h <= kp.hav_max;
 }
 
-// KFN: kernel function (hcgrid_set_kernel), 0 Gaussian, 1 tapered sinc -- a template parameter so
+// Elliptical Gaussian from the fp32 pair arithmetic (series path: support radius and longitude half-window
+// <= 0.05 rad).  With dx, dy the exact coordinate differences (rad), C = cos(lat_c) cos(lat_s) (the strip's
+// polynomial in dy) and B = 4 sin^2(dx / 2) (series):
+//     x = cos(lat_s) sin dx          = C sin(dx) / cos(lat_c)
+//     y = sin dy + 2 sin(lat_c) cos(lat_s) sin^2(dx / 2) = sin(dy) + (tan(lat_c) / 2) C B
+//     (d sin(beta - PA))^2 = (x cos PA - y sin PA)^2 (d / sin d)^2,  (d / sin d)^2 = 1 + d^2/3 + ... = 1 + h4/3 + O(d^4)
+// sin z = z (1 - z^2/6 + z^4/120): next term 1.6e-12 relative at 0.05 rad.  icc = 1 / cos(lat_c), th = tan(lat_c) / 2.
+__device__ __forceinline__ bool pair32_elliptical(const Rec32& r, const TaskConst& tc, float icc, float th,
+                                                  const KernelParams& kp, float& w) {
+    const float dx = (float)(int)(r.xi - tc.xc0) * tc.qx;
+    const float dy = (float)(int)(r.yi - tc.yc) * tc.qy;
+    const float u = dy * dy;
+    const float u2 = u * fmaf(u, -1.0f / 12.0f, 1.0f);
+    const float C = fmaf(dy, fmaf(dy, fmaf(dy, tc.c3, tc.c2), tc.c1), tc.c0);
+    const float v = dx * dx;
+    const float B = v * fmaf(v, -1.0f / 12.0f, 1.0f);
+    const float CB = C * B;
+    const float h4 = CB + u2;
+    const float sdx = dx * fmaf(v, fmaf(v, 1.0f / 120.0f, -1.0f / 6.0f), 1.0f);
+    const float sdy = dy * fmaf(u, fmaf(u, 1.0f / 120.0f, -1.0f / 6.0f), 1.0f);
+    const float x = C * sdx * icc;
+    const float y = fmaf(th, CB, sdy);
+    const float t = x * kp.ecp - y * kp.esp;
+    const float e2 = fmaf(h4, fmaf(h4, tc.k2, tc.k1), t * t * fmaf(h4, 1.0f / 3.0f, 1.0f) * kp.ek2);
+    w = ex2_approx(e2);
+    return h4 <= tc.h4max;
+}
+
+// KFN: kernel function (hcgrid_set_kernel), 0 Gaussian, 1 tapered sinc, 2 elliptical Gaussian -- a template parameter so
 // that the Gaussian instantiations carry none of the other's code.
 template <bool PAIR64, typename AccT, bool VEC4, int KFN>
 __global__ void __launch_bounds__(256)
@@ -106,13 +151,20 @@ conv_general(const ConvArgs a) {
 
     // cell constants
     TaskConst tc;
-    double clon_deg = 0.0, clat_deg = 0.0, ccos = 0.0;
+    double clon_deg = 0.0, clat_deg = 0.0, ccos = 0.0, csin = 0.0;
+    float icc = 0.0f, th = 0.0f;                    // elliptical Gaussian, fp32 pairs: 1 / cos(lat_c), tan(lat_c) / 2
     if (PAIR64) {
         clon_deg = __dadd_rn(st.lon0_deg, __dmul_rn((double)ix, st.dlon_deg));   // no FMA (SURVEY 8c fp64 pin)
         clat_deg = st.lat_deg;
         ccos = cos(clat_deg * kDeg2Rad);
+        if (KFN == 2) csin = sin(clat_deg * kDeg2Rad);
     } else {
         tc = make_task_const(a, st, ix);
+        if (KFN == 2) {
+            const double cl = cos(st.lat);
+            icc = (float)(1.0 / cl);
+            th = (float)(0.5 * sin(st.lat) / cl);
+        }
     }
 
     for (int ch0 = 0; ch0 < nchan; ch0 += 256) {
@@ -136,8 +188,8 @@ conv_general(const ConvArgs a) {
                     if (PAIR64) {
                         const Rec64 r = ((const Rec64*)a.rec)[sa + i];
                         double wd;
-                        hit = a.small64 ? pair64_small<KFN>(r, clon_deg, clat_deg, ccos, a.kp, wd)
-                                        : pair64<KFN>(r, clon_deg, clat_deg, ccos, a.kp, wd);
+                        hit = a.small64 ? pair64_small<KFN>(r, clon_deg, clat_deg, ccos, csin, a.kp, wd)
+                                        : pair64<KFN>(r, clon_deg, clat_deg, ccos, csin, a.kp, wd);
                         wq = (AccT)(wd * (double)r.q);
                         idx = r.idx;
                     } else {
@@ -145,8 +197,12 @@ conv_general(const ConvArgs a) {
                         Rec32 r;
                         r.xi = raw.x; r.yi = raw.y; r.idx = raw.z; r.q = __uint_as_float(raw.w);
                         float wf, e2;
-                        hit = pair32(r, tc, wf, &e2);
-                        if (KFN != 0) wf = tapered_sinc32(e2, a.kp);
+                        if (KFN == 2) {
+                            hit = pair32_elliptical(r, tc, icc, th, a.kp, wf);
+                        } else {
+                            hit = pair32(r, tc, wf, &e2);
+                            if (KFN == 1) wf = tapered_sinc32(e2, a.kp);
+                        }
                         wq = (AccT)(wf * r.q);
                         idx = r.idx;
                     }
@@ -231,7 +287,8 @@ int launch_conv_general(hcgrid_ctx* c, const ConvArgs& a0, bool pair_f64, bool o
 #define HCG_LAUNCH(P, T, V)                                                        \
     do {                                                                           \
         if (a.kp.ktype == 0) conv_general<P, T, V, 0><<<blocks, threads, 0, st>>>(a); \
-        else conv_general<P, T, V, 1><<<blocks, threads, 0, st>>>(a);              \
+        else if (a.kp.ktype == 1) conv_general<P, T, V, 1><<<blocks, threads, 0, st>>>(a); \
+        else conv_general<P, T, V, 2><<<blocks, threads, 0, st>>>(a);              \
     } while (0)
     if (out_double) {
         if (vec4) HCG_LAUNCH(true, double, true); else HCG_LAUNCH(true, double, false);

@@ -61,6 +61,7 @@ conv1_tile_f32(const TileArgs a) {
         ring_lo[j] = r0.y;
         nring[j] = j < nrows ? r0.z : 0;
         tc.cc[j] = __int_as_float(r0.w);
+        if (KFN == 2) tc.sh[j] = 0.5f * __int_as_float(r1.x) * a.isk;
         if (j == 0) {
             tc.yc0 = (uint32_t)r0.x;
             tc.cc0 = __int_as_float(r0.w);
@@ -79,6 +80,7 @@ conv1_tile_f32(const TileArgs a) {
     tc.sxk = a.sxk; tc.syk = a.syk; tc.duk = a.duk; tc.dyk = a.dyk;
     tc.a12 = a.a12; tc.hmax = a.hmax;
     tc.ts1 = a.ts1; tc.tg2 = a.tg2;
+    tc.ecp = a.ecp; tc.esp = a.esp; tc.erk = a.erk;
 
     float W[NC], S_[NC];
     int cnt[NC];
@@ -213,30 +215,32 @@ static cudaError_t launch_shape(const TileArgs& a, int mode, bool counts, cudaSt
     return cudaGetLastError();
 }
 
-// Tapered sinc (KFN 1): series mode 2 only (valid wherever the tile kernel is), three shapes.
-template <int GX, int GY>
-static cudaError_t launch_shape_sinc(const TileArgs& a, bool counts, cudaStream_t st) {
+// Tapered sinc (KFN 1) and elliptical Gaussian (KFN 2): series mode 2 only (valid wherever the tile kernel is),
+// three shapes.
+template <int GX, int GY, int KFN>
+static cudaError_t launch_shape_kfn(const TileArgs& a, bool counts, cudaStream_t st) {
     const unsigned blocks = a.split > 1 ? (unsigned)a.ntiles : (unsigned)((a.ntiles + kTileWarps - 1) / kTileWarps);
     const int threads = (a.split > 1 ? a.split : kTileWarps) * 32;
     if (counts) {
-        if (a.split > 1) conv1_tile_f32<GX, GY, 2, true, true, 1><<<blocks, threads, 0, st>>>(a);
-        else conv1_tile_f32<GX, GY, 2, true, false, 1><<<blocks, threads, 0, st>>>(a);
+        if (a.split > 1) conv1_tile_f32<GX, GY, 2, true, true, KFN><<<blocks, threads, 0, st>>>(a);
+        else conv1_tile_f32<GX, GY, 2, true, false, KFN><<<blocks, threads, 0, st>>>(a);
     } else {
-        if (a.split > 1) conv1_tile_f32<GX, GY, 2, false, true, 1><<<blocks, threads, 0, st>>>(a);
-        else conv1_tile_f32<GX, GY, 2, false, false, 1><<<blocks, threads, 0, st>>>(a);
+        if (a.split > 1) conv1_tile_f32<GX, GY, 2, false, true, KFN><<<blocks, threads, 0, st>>>(a);
+        else conv1_tile_f32<GX, GY, 2, false, false, KFN><<<blocks, threads, 0, st>>>(a);
     }
     return cudaGetLastError();
 }
 
 static const int kShapes[][2] = {{1, 1}, {2, 1}, {4, 1}, {8, 1}, {2, 2}, {4, 2}, {8, 2}, {4, 4}};
-static bool sinc_shape_built(int gx, int gy) { return (gx == 1 && gy == 1) || (gx == 2 && gy == 2) || (gx == 4 && gy == 2); }
+static bool kfn_shape_built(int gx, int gy) { return (gx == 1 && gy == 1) || (gx == 2 && gy == 2) || (gx == 4 && gy == 2); }
 
 // Instruction-count model of one tile: warp instructions per cell.
 static double shape_cost(int gx, int gy, int mode, bool counts, double cw, double ch, double two_r,
-                         double ring_sp, double cand_per_cell, bool sinc = false) {
+                         double ring_sp, double cand_per_cell, int kfn = 0) {
     const double infl = (two_r + (gx - 1) * cw) / two_r * (two_r + 2.0 * ring_sp + (gy - 1) * ch) / (two_r + 2.0 * ring_sp);
     const double per_iter = 18.0 + (mode >= 1 ? 4.0 : 2.0) * gx + (mode >= 1 ? 5.0 : 3.0) * gy +
-                            (5.0 + (counts ? 1.0 : 0.0) + (mode == 2 ? 2.0 : 0.0) + (sinc ? 45.0 : 0.0)) * gx * gy;
+                            (5.0 + (counts ? 1.0 : 0.0) + (mode == 2 ? 2.0 : 0.0) + (kfn == 1 ? 45.0 : kfn == 2 ? 6.0 : 0.0)) * gx * gy +
+                            (kfn == 2 ? 5.0 * (gx + gy) : 0.0);
     const double iters = cand_per_cell * infl / 32.0 + 0.5;
     const double overhead = 150.0 + 14.0 * gy + 8.0 * gx * gy;
     // 16-cell tiles need ~100 registers per thread; measured on B200 they run 15-25 % slower than
@@ -279,8 +283,8 @@ int launch_conv_tile(hcgrid_ctx* c, int64_t n, float* cube, float* wmap, int32_t
     const Region& rg = c->region;
     const KernelParams& kp = c->kp;
     const int nx = c->strip_cells, ny = c->nstrip;
-    const bool sinc = kp.ktype == HCGRID_KERNEL_TAPERED_SINC;
-    const int mode = sinc ? 2 : tile_series_mode(c);
+    const int kfn = kp.ktype;            // 0 Gaussian, 1 tapered sinc, 2 elliptical Gaussian
+    const int mode = kfn != 0 ? 2 : tile_series_mode(c);
 
     // tile shape: forced by the options or chosen by the instruction-count model
     int gx = c->opt_coarsen, gy = c->opt_coarsen_y;
@@ -296,9 +300,9 @@ int launch_conv_tile(hcgrid_ctx* c, int64_t n, float* cube, float* wmap, int32_t
             if ((gx != 0 && s[0] != gx) || (gy != 0 && s[1] != gy)) continue;
             if (s[0] > nx && s[0] > 1) continue;
             if (s[1] > ny && s[1] > 1) continue;
-            if (sinc && !sinc_shape_built(s[0], s[1])) continue;
+            if (kfn != 0 && !kfn_shape_built(s[0], s[1])) continue;
             const double cost = shape_cost(s[0], s[1], mode, counts != nullptr, c->cell_width_sky,
-                                           std::fabs(c->car_dlat), two_r, ring_sp, cand, sinc);
+                                           std::fabs(c->car_dlat), two_r, ring_sp, cand, kfn);
             if (cost < best) { best = cost; bx = s[0]; by = s[1]; }
         }
         if (best == 1e300)
@@ -330,9 +334,14 @@ int launch_conv_tile(hcgrid_ctx* c, int64_t n, float* cube, float* wmap, int32_t
 
     cudaError_t e = cudaSuccess;
     bool built = false;
-    if (sinc) {
+    if (kfn == HCGRID_KERNEL_TAPERED_SINC) {
         a.ts1 = kp.ts1; a.tg2 = kp.tg2;
-#define HCG_SHAPE(X, Y) if (gx == X && gy == Y) { built = true; e = launch_shape_sinc<X, Y>(a, counts != nullptr, st); }
+#define HCG_SHAPE(X, Y) if (gx == X && gy == Y) { built = true; e = launch_shape_kfn<X, Y, 1>(a, counts != nullptr, st); }
+        HCG_SHAPE(1, 1); HCG_SHAPE(2, 2); HCG_SHAPE(4, 2);
+#undef HCG_SHAPE
+    } else if (kfn == HCGRID_KERNEL_ELLIPTICAL_GAUSS) {
+        a.ecp = kp.ecp; a.esp = kp.esp; a.erk = (float)(kp.ell_k / kp.inv2s2);
+#define HCG_SHAPE(X, Y) if (gx == X && gy == Y) { built = true; e = launch_shape_kfn<X, Y, 2>(a, counts != nullptr, st); }
         HCG_SHAPE(1, 1); HCG_SHAPE(2, 2); HCG_SHAPE(4, 2);
 #undef HCG_SHAPE
     } else {

@@ -95,19 +95,26 @@ struct Region {            // what of the sphere the target can reach (host + de
     double sx32, sy32;     // fixed-point units per radian (lon, lat): 2^32 over a span >= wx / wy (target.cu)
 };
 
+constexpr double kF32RadiusMax = 0.004;   // rad: largest support radius of the fp32 pair arithmetic (target.cu)
+
 struct KernelParams {      // per-context constants of the pair arithmetic
     double sigma, radius;              // rad
     double inv2s2;                     // 1 / (2 sigma^2)
     double hav_max;                    // sin^2(R/2)
     float h4max;                       // 4 sin^2(R/2), rounded to fp32
     float k1, k2;                      // exponent = h4 * (k1 + k2 * h4): -log2e/(2 sigma^2) * (1, 1/12)
-    // kernel function (hcgrid_set_kernel): 0 Gaussian, 1 tapered sinc
+    // kernel function (hcgrid_set_kernel): 0 Gaussian, 1 tapered sinc, 2 elliptical Gaussian
     //   sinc(d / (b sigma)) exp(-(d / (a sigma))^2),  sinc(x) = sin(pi x) / (pi x)
     int ktype;
     double inv_a2s2, pi_bs;            // 1 / (a sigma)^2,  pi / (b sigma)
     float tg2, ts1;                    // fp32 path, from t = -exponent above = d^2 log2e / (2 sigma^2):
                                        // taper = ex2(-t * tg2), tg2 = 2 / a^2; sinc argument = ts1 * sqrt(t),
                                        // ts1 = pi sqrt(2 ln 2) / b
+    // 2 elliptical Gaussian (reading c21): sigma along the axis at position angle PA (from north through
+    //   east), ratio * sigma across it; exponent = d^2 / (2 sigma^2) + (d sin(beta - PA))^2 * ell_k
+    double ell_k;                      // 1 / (2 (ratio sigma)^2) - 1 / (2 sigma^2)
+    double ell_cp, ell_sp;             // cos PA, sin PA
+    float ek2, ecp, esp;               // fp32 path: -log2e * ell_k, cos PA, sin PA
 };
 
 // ---------------------------------------------------------------- host-side helpers
@@ -142,7 +149,8 @@ struct hcgrid_ctx {
     bool is_car = false;
     int64_t ncell = 0;
     int32_t nstrip = 0, strip_cells = 0, kmax = 0;
-    bool f32_series_ok = true;      // small-angle series valid over the whole target
+    bool small_series_ok = true;    // small-angle series valid over the whole target (R, longitude half-window <= 0.05 rad)
+    bool f32_series_ok = true;      // ... and the fp32 pair arithmetic resolves the support boundary to 1e-9 rad (R <= kF32RadiusMax)
     double cell_width_sky = 0.0;    // min over strips of |du| cos(lat), rad (coarsening choice)
     hcg::Region region{};
     hcg::DevBuf d_strips, d_wins, d_winsf, d_rowsf, d_cell_lon, d_cell_lat;

@@ -26,6 +26,7 @@ struct TileArgs {
     float a12;                  // 1 / (12 kappa): series coefficient in scaled units
     float hmax;                 // kappa * 4 sin^2(R/2)  (series modes)  or  kappa * R^2 (flat mode)
     float ts1, tg2;             // tapered sinc (KFN 1): sinc argument = ts1 sqrt(e), taper = ex2(-e tg2)
+    float ecp, esp, erk;        // elliptical Gaussian (KFN 2): cos PA, sin PA, (sigma_1 / sigma_2)^2 - 1
 };
 
 template <int GY>
@@ -37,6 +38,8 @@ struct TileConst {
     float a12, hmax;
     float hm;                   // hmax, or -1 for a lane that is past the end of the stream
     float ts1, tg2;             // KFN 1 only
+    float ecp, esp, erk;        // KFN 2 only
+    float sh[GY];               // KFN 2 only: sin(lat_c) / (2 sqrt(kappa)) of the tile's rows
 };
 
 // Tapered sinc from e = kappa d^2 (the Gaussian's base-2 exponent): sinc(ts1 sqrt(e)) ex2(-e tg2).
@@ -63,6 +66,11 @@ __device__ __forceinline__ float tile_tapered_sinc(float e, float ts1, float tg2
 // MODE 1 "series": 4 hav(d) = u(1-u/12) + C v(1-v/12) for the test, weight from the same;
 // MODE 2 "full": as 1, plus d^2 = h(1 + h/12) for the weight.
 // KFN 0: Gaussian, w = ex2(-e); KFN 1: tapered sinc of the same e (hcgrid_set_kernel).
+// KFN 2: elliptical Gaussian (reading c21; MODE 2 only), w = ex2(-(e + erk t^2 (1 + h / (3 kappa)))) with
+//   t = sqrt(kappa) (x cos PA - y sin PA),  x = cos(lat_s) sin dx,  y = sin dy + sin(lat_c) cos(lat_s) 2 sin^2(dx / 2)
+// -- x, y the sample's direction along the cell's east and north, (d sin(beta - PA))^2 = (x cos PA - y sin PA)^2
+// (d / sin d)^2, (d / sin d)^2 = 1 + d^2 / 3 + ...; in the scaled units sin z = z (1 - 2 a12 z^2 + 1.2 a12^2 z^4) and
+// 2 sin^2(dx / 2) = V / (2 kappa).
 template <int GX, int GY, int MODE, bool COUNTS, int KFN = 0>
 __device__ __forceinline__ void tile_pairs(const uint4 raw, const TileConst<GY>& tc, float (&W)[GX * GY],
                                            float (&S)[GX * GY], int (&cnt)[GX * GY]) {
@@ -72,11 +80,14 @@ __device__ __forceinline__ void tile_pairs(const uint4 raw, const TileConst<GY>&
     const float dy0 = (float)(int)(raw.y - tc.yc0) * tc.syk;
     const float cs = fmaf(dy0, fmaf(dy0, fmaf(dy0, tc.p3, tc.p2), tc.p1), tc.cc0);
     float V[GX], U[GY], C[GY];
+    float X[GX], Y[GY], SH[GY];                    // KFN 2: x cos PA; sin(dy) sin PA; sin(lat_c) cos(lat_s) sin PA / 2, scaled
+    const float a6 = 2.0f * tc.a12, a120 = 1.2f * tc.a12 * tc.a12;
 #pragma unroll
     for (int i = 0; i < GX; ++i) {
         const float dx = i == 0 ? dx0 : fmaf(-(float)i, tc.duk, dx0);
         const float v = dx * dx;
         V[i] = MODE >= 1 ? v * fmaf(v, -tc.a12, 1.0f) : v;
+        if (KFN == 2) X[i] = dx * fmaf(v, fmaf(v, a120, -a6), 1.0f) * (cs * tc.ecp);
     }
 #pragma unroll
     for (int j = 0; j < GY; ++j) {
@@ -84,14 +95,22 @@ __device__ __forceinline__ void tile_pairs(const uint4 raw, const TileConst<GY>&
         const float u = dy * dy;
         U[j] = MODE >= 1 ? u * fmaf(u, -tc.a12, 1.0f) : u;
         C[j] = tc.cc[j] * cs;
+        if (KFN == 2) {
+            Y[j] = dy * fmaf(u, fmaf(u, a120, -a6), 1.0f) * tc.esp;
+            SH[j] = tc.sh[j] * (cs * tc.esp);
+        }
     }
 #pragma unroll
     for (int j = 0; j < GY; ++j) {
 #pragma unroll
         for (int i = 0; i < GX; ++i) {
             const float h = fmaf(C[j], V[i], U[j]);
-            const float e = MODE == 2 ? h * fmaf(h, tc.a12, 1.0f) : h;
-            const float w = KFN == 0 ? ex2_approx(-e) : tile_tapered_sinc(fmaxf(e, 0.0f), tc.ts1, tc.tg2);
+            float e = MODE == 2 ? h * fmaf(h, tc.a12, 1.0f) : h;
+            if (KFN == 2) {
+                const float t = fmaf(-SH[j], V[i], X[i] - Y[j]);
+                e = fmaf(tc.erk * (t * t), fmaf(h, 4.0f * tc.a12, 1.0f), e);
+            }
+            const float w = KFN == 1 ? tile_tapered_sinc(fmaxf(e, 0.0f), tc.ts1, tc.tg2) : ex2_approx(-e);
             // predicated accumulate, spelled out so the count stays one predicated add
             if (COUNTS)
                 asm("{\n\t.reg .pred p;\n\t"

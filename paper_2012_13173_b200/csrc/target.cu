@@ -200,7 +200,12 @@ static int finish_target(hcgrid_ctx* c, const std::vector<HostStrip>& hs, int st
     c->cell_width_sky = strip_cells > 1 ? cw : 0.0;
     // small-angle series of the fp32 pair arithmetic: valid while R and the widest
     // longitude half-window stay below 0.05 rad (dropped x^6/360 term < 2e-8 relative)
-    c->f32_series_ok = !pole && R <= 0.05 && dlmax <= 0.05;
+    c->small_series_ok = !pole && R <= 0.05 && dlmax <= 0.05;
+    // The fp32 pair arithmetic itself delivers 4 sin^2(d/2) to ~4 ulp (2.4e-7 relative), i.e. d to 1.2e-7 relative:
+    // it settles "d <= R" to better than the 1e-9 rad the count parity allows (reading c4) only while
+    // R <= 0.004 rad (0.23 deg; the paper's five workloads have R <= 0.0013 rad).  Wider kernels take the fp64
+    // pair arithmetic (series form where valid) with the accumulation of the chosen mode.
+    c->f32_series_ok = c->small_series_ok && R <= kF32RadiusMax;
 
     HCG_CUDA(c, c->d_strips.ensure(st.size() * sizeof(Strip)));
     HCG_CUDA(c, cudaMemcpy(c->d_strips.p, st.data(), st.size() * sizeof(Strip), cudaMemcpyHostToDevice));

@@ -109,7 +109,7 @@ def test_tc_kernel_empty_input_and_empty_tiles(oracle):
     assert np.all(np.isnan(cube)) and np.all(wmap == 0) and np.all(cnt == 0)
 
 
-@pytest.mark.parametrize("radius_deg,sigma_deg", [(0.1, 0.04), (0.2, 0.08), (1.5, 0.5)])
+@pytest.mark.parametrize("radius_deg,sigma_deg", [(0.1, 0.04), (0.2, 0.08), (0.225, 0.05)])
 def test_tc_kernel_series_modes(oracle, radius_deg, sigma_deg):
     """Wider kernels switch the pair arithmetic to the series / full modes; several ring-table passes."""
     from paper_2012_13173_b200 import binding
@@ -128,7 +128,7 @@ def test_tc_kernel_series_modes(oracle, radius_deg, sigma_deg):
 
 
 def test_tc_kernel_many_rings_per_tile(oracle):
-    """nside 8192 under a 6' kernel: a tile's ring range exceeds one 128-entry table pass."""
+    """nside 16384 (the largest) under a 4.5' kernel: a tile's ring range (~200) exceeds one 128-entry table pass."""
     from paper_2012_13173_b200 import binding
     rng = np.random.default_rng(79)
     n = 30000
@@ -136,7 +136,7 @@ def test_tc_kernel_many_rings_per_tile(oracle):
     w.lon = 100.0 + rng.uniform(-0.5, 0.5, n)
     w.lat = -10.0 + rng.uniform(-0.5, 0.5, n)
     w.values = rng.normal(size=(n, 32)).astype(np.float32)
-    w.sigma_deg, w.radius_deg, w.nside = 6.0 / 60, 18.0 / 60, 8192
+    w.sigma_deg, w.radius_deg, w.nside = 4.5 / 60, 13.5 / 60, 16384
     w.target = workloads.CarTarget(20, 12, 99.8, -10.15, 2.0 / 60, -(-2.0) / 60)
     ref = run_oracle(oracle, w)
     cube, wmap, cnt, st = run_gpu(w, "f32", {binding.OPT_KERNEL: 7})

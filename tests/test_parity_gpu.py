@@ -173,7 +173,37 @@ def test_cube_kernel_falls_back_for_odd_channel_counts(oracle):
     assert st["kernel"] == 8                     # 256 channels: the tensor-core cube kernel
 
 
-@pytest.mark.parametrize("radius_deg,sigma_deg", [(0.1, 0.04), (0.2, 0.08), (1.5, 0.5)])
+def test_wide_kernels_take_the_fp64_pair_arithmetic(oracle):
+    """R > 0.004 rad: fp32 arithmetic can no longer settle d <= R to the 1e-9 rad of the count bar (d to 1.2e-7
+    relative), so the fp32 mode keeps its fp32 sums but tests and weighs the pairs in fp64; forcing an fp32-pair
+    kernel there is refused."""
+    from paper_2012_13173_b200 import binding
+    rng = np.random.default_rng(771)
+    n = 6000
+    w = workloads.make(1, 1.0)
+    w.lon = 200.0 + rng.uniform(-2.0, 2.0, n)
+    w.lat = 40.0 + rng.uniform(-2.0, 2.0, n)
+    w.sigma_deg, w.radius_deg, w.nside = 0.5, 1.5, 256
+    w.target = workloads.CarTarget(23, 19, 199.0, 39.1, 0.09, 0.1)
+    for nchan in (1, 8):
+        w.values = rng.normal(size=(n, nchan)).astype(np.float32)
+        ref = run_oracle(oracle, w)
+        cube, wmap, cnt, st = run_gpu(w, "f32")
+        assert st["kernel"] == 4
+        compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F32)
+    for forced in (binding.KERNEL_TILE, binding.KERNEL_CUBE, binding.KERNEL_CUBE_TC):
+        with pytest.raises(binding.HCGridError):
+            run_gpu(w, "f32", {binding.OPT_KERNEL: forced})
+    # just below the limit (0.229 deg) the tile kernel still runs
+    w.sigma_deg, w.radius_deg = 0.06, 0.229
+    w.values = rng.normal(size=(n, 1)).astype(np.float32)
+    ref = run_oracle(oracle, w)
+    cube, wmap, cnt, st = run_gpu(w, "f32")
+    assert st["kernel"] == 6
+    compare(cube, wmap, cnt, ref, w.sigma_deg, w.radius_deg, TOL_F32)
+
+
+@pytest.mark.parametrize("radius_deg,sigma_deg", [(0.1, 0.04), (0.2, 0.08), (0.225, 0.05)])
 def test_tile_series_modes(oracle, radius_deg, sigma_deg):
     """Wider kernels switch the tile kernel's pair arithmetic to the series / full modes."""
     rng = np.random.default_rng(77)
@@ -552,17 +582,17 @@ def test_all_sky_target_starting_at_minus_180(oracle, kernel, precision):
     put to the distance test stays a small multiple of the hits on both halves of the sky."""
     from paper_2012_13173_b200 import binding
     rng = np.random.default_rng([13173, 808])
-    n = 150000
+    n = 600000
     lon = rng.uniform(0.0, 360.0, n)
     lat = np.rad2deg(np.arcsin(rng.uniform(np.sin(np.deg2rad(-62.0)), np.sin(np.deg2rad(62.0)), n)))
     val = rng.standard_normal((n, 1)).astype(np.float32)
-    sigma, radius = 0.4, 1.2
+    sigma, radius = 0.075, 0.225                    # 3.9e-3 rad: the widest kernels the fp32 pair arithmetic takes
     tgt = workloads.CarTarget(360, 61, -180.0, -60.0, 1.0, 2.0)
     cl, cb = tgt.cell_centers()
     ref = oracle.grid(sigma, radius, cl, cb, lon, lat, val, None)
     pairs = {}
     for lon0 in (-180.0, 0.0, 97.0):                # the same 360 cells per row, listed from three starting points
-        g = binding.HCGrid(sigma, radius, 256, precision=precision)
+        g = binding.HCGrid(sigma, radius, 1024, precision=precision)
         g.set_option(binding.OPT_PROFILE, 1)
         if kernel:
             g.set_option(binding.OPT_KERNEL, kernel)
