@@ -201,6 +201,8 @@ def run_product(args):
     elif args.kernel_function == "elliptical":
         g.set_kernel(binding.KERNEL_ELLIPTICAL_GAUSS, 0.5, 30.0)
     if args.explicit_cells:                            # the same cells handed over one by one (hcgrid_set_target_cells)
+        if args.per_cell_path:
+            g.set_option(binding.OPT_CELLS_AS_GRID, 0)     # do not recognise the grid: time the per-cell path itself
         cl, cb = t.cell_centers()
         g.set_target_cells(torch.from_numpy(cl).to(dev), torch.from_numpy(cb).to(dev))
     else:
@@ -368,7 +370,8 @@ def run_product(args):
                    "e2e_path": "hcgrid_grid_host, pinned buffers; inputs of 64 MB or more are copied in 4 pieces and gridded as they arrive", "per_rank": "one independent problem" if units_total is None else "a band of target rows + its samples (rank 0's figures in roofline / stages)",
                    "outputs": "datacube + weight map (count output off in the timed calls)",
                    "kernel_function": args.kernel_function,
-                   "target": "per-cell lon/lat (hcgrid_set_target_cells)" if args.explicit_cells else "CAR parameters"},
+                   "target": ("per-cell lon/lat (hcgrid_set_target_cells), grid recognition " + ("off" if args.per_cell_path else "on"))
+                             if args.explicit_cells else "CAR parameters"},
         "kernel_evals_per_s": n_hit * world * args.steps / (ms_total * 1e-3),
         "conv_kernel": {"us": t_conv * 1e6, "cell_channels_per_s": ncell * nchan / t_conv,
                         "kernel_evals_per_s": n_hit / t_conv,
@@ -435,6 +438,8 @@ def main():
                          "the elliptical Gaussian (ratio 0.5, position angle 30 deg)")
     ap.add_argument("--explicit-cells", action="store_true",
                     help="hand the target over as per-cell lon/lat (hcgrid_set_target_cells) instead of CAR parameters")
+    ap.add_argument("--per-cell-path", action="store_true",
+                    help="with --explicit-cells: switch the grid recognition off (HCGRID_OPT_CELLS_AS_GRID 0)")
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per launch of the convolution kernel from the committed ncu capture")
     args = ap.parse_args()

@@ -73,6 +73,18 @@ enum {
     HCGRID_OPT_HOST_CHUNKS = 9,  /* hcgrid_grid_host: pieces the samples are copied and gridded in (copy of piece
                                     k+1 overlaps the gridding of piece k); 1 = one copy, one hcgrid_grid; 0 = auto
                                     (4 from 64 MB of input) */
+    HCGRID_OPT_CELLS_AS_GRID = 10, /* hcgrid_set_target_cells: 1 (default) = cells that are a plate-carree grid listed
+                                    row by row (lon0 + ix*dlon, lat0 + iy*dlat: what a WCS CAR header expands to) are
+                                    recognised and take the plate-carree path; in fp64 mode only when those two
+                                    expressions reproduce every centre bit for bit, in fp32 mode to 1e-10 deg;
+                                    0 = always the per-cell path.  Set before hcgrid_set_target_cells. */
+    HCGRID_OPT_GRAPH = 11,       /* replay of repeated calls: an hcgrid_grid call with the same arrays, sizes, options
+                                    and target as the one before it is captured as a CUDA graph, and every further
+                                    identical call is one graph launch (the arrays' contents may change, their
+                                    addresses and sizes may not: any other call runs eagerly and starts over).
+                                    -1 = auto (default): inputs of up to 2^21 samples, which are bound by launch
+                                    gaps; 0 = never; 1 = any size.  Not used with HCGRID_OPT_PROFILE or while an
+                                    accumulation is open. */
     HCGRID_OPT_PREORDER = 8      /* how S' is ordered: 1 = radix sort of (key, n); 2 = counting sort into the
                                     bin table (same S', bit for bit); 0 = auto (counting up to 10 samples per bin) */
 };
@@ -92,6 +104,8 @@ typedef struct {
     int32_t preorder;         /* pre-ordering used: 1 radix sort, 2 counting sort             */
     int64_t n_hit;            /* PROFILE + count output: pairs (cell, sample) with d <= R = sum of the counts
                                  ("kernel evaluations"); -1 otherwise                            */
+    int32_t graph;            /* 1: the call was replayed from (or captured into) a CUDA graph (HCGRID_OPT_GRAPH) */
+    int32_t pad_;
     int64_t n_pairs_tested;   /* PROFILE, tile and strip kernels (kernel 1..6): pairs the kernel put to the distance
                                  test (candidate stream length x cells of every tile or task); -1 otherwise     */
 } hcgrid_stats;
@@ -134,7 +148,8 @@ int hcgrid_set_kernel(hcgrid_ctx* ctx, int32_t kernel_type, double a, double b);
  * not zero.  Builds the per-row search tables on the device (synchronises the device). */
 int hcgrid_set_target_car(hcgrid_ctx* ctx, int32_t nx, int32_t ny, double lon0_deg,
                           double lat0_deg, double dlon_deg, double dlat_deg);
-/* Target = arbitrary cells; lon_deg/lat_deg are DEVICE arrays [ncell] (copied). */
+/* Target = arbitrary cells; lon_deg/lat_deg are DEVICE arrays [ncell] (copied; synchronises the stream).  Cells
+ * that form a plate-carree grid are recognised (HCGRID_OPT_CELLS_AS_GRID) and gridded like hcgrid_set_target_car's. */
 int hcgrid_set_target_cells(hcgrid_ctx* ctx, int64_t ncell, const double* lon_deg,
                             const double* lat_deg, void* stream);
 

@@ -20,6 +20,8 @@ _lib = None
 F32, F64 = 0, 1
 OPT_PROFILE, OPT_SUBPIX_BITS, OPT_COARSEN, OPT_KERNEL, OPT_WARPS_PER_SM, OPT_COARSEN_Y, OPT_SPLIT, OPT_PREORDER = 1, 2, 3, 4, 5, 6, 7, 8
 OPT_HOST_CHUNKS = 9
+OPT_CELLS_AS_GRID = 10
+OPT_GRAPH = 11
 PREORDER_AUTO, PREORDER_RADIX, PREORDER_COUNTING = 0, 1, 2
 KERNEL_AUTO, KERNEL_SIMPLE, KERNEL_F64PAIR, KERNEL_GENERAL, KERNEL_STAGED, KERNEL_TILE, KERNEL_CUBE, KERNEL_CUBE_TC = 0, 1, 2, 3, 4, 5, 6, 7
 
@@ -47,7 +49,8 @@ class Stats(ctypes.Structure):
                 ("us_pixelise", ctypes.c_float), ("us_sort", ctypes.c_float), ("us_tables", ctypes.c_float),
                 ("us_pack", ctypes.c_float), ("us_convolve", ctypes.c_float), ("us_total", ctypes.c_float),
                 ("split", ctypes.c_int32), ("preorder", ctypes.c_int32),
-                ("n_hit", ctypes.c_int64), ("n_pairs_tested", ctypes.c_int64)]
+                ("n_hit", ctypes.c_int64), ("graph", ctypes.c_int32), ("pad_", ctypes.c_int32),
+                ("n_pairs_tested", ctypes.c_int64)]
 
     def asdict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

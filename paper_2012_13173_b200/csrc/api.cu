@@ -94,13 +94,20 @@ int hcgrid_destroy(hcgrid_ctx* c) {
     for (auto& ev : c->ev_chunk) if (ev) cudaEventDestroy(ev);
     if (c->st_copy) cudaStreamDestroy(c->st_copy);
     if (c->st_comp) cudaStreamDestroy(c->st_comp);
+    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    if (c->st_cap) cudaStreamDestroy(c->st_cap);
     delete c;
     return HCGRID_OK;
 }
 
 int hcgrid_set_option(hcgrid_ctx* c, int option, int64_t value) {
     if (!c) return HCGRID_ERR_INVALID_ARG;
+    ++c->config_gen;
     switch (option) {
+        case HCGRID_OPT_GRAPH:
+            if (value < -1 || value > 1) return fail(c, HCGRID_ERR_INVALID_ARG, "graph must be -1 (auto), 0 or 1");
+            c->opt_graph = (int)value;
+            break;
         case HCGRID_OPT_PROFILE: c->opt_profile = value != 0; break;
         case HCGRID_OPT_SUBPIX_BITS:
             if (value < -1 || value > 6) return fail(c, HCGRID_ERR_INVALID_ARG, "subpix bits must be -1 (auto) or 0..6");
@@ -131,6 +138,10 @@ int hcgrid_set_option(hcgrid_ctx* c, int option, int64_t value) {
             if (value < 0 || value > 16) return fail(c, HCGRID_ERR_INVALID_ARG, "host chunks must be 0 (auto) or 1..16");
             c->opt_host_chunks = (int)value;
             break;
+        case HCGRID_OPT_CELLS_AS_GRID:
+            if (value < 0 || value > 1) return fail(c, HCGRID_ERR_INVALID_ARG, "cells-as-grid must be 0 or 1");
+            c->opt_cells_as_grid = (int)value;
+            break;
         case HCGRID_OPT_PREORDER:
             if (value < 0 || value > 2) return fail(c, HCGRID_ERR_INVALID_ARG, "preorder must be 0 (auto), 1 or 2");
             c->opt_preorder = (int)value;
@@ -142,6 +153,7 @@ int hcgrid_set_option(hcgrid_ctx* c, int option, int64_t value) {
 
 int hcgrid_set_kernel(hcgrid_ctx* c, int32_t kernel_type, double a, double b) {
     if (!c) return HCGRID_ERR_INVALID_ARG;
+    ++c->config_gen;
     if (c->acc_nchan != 0)
         return fail(c, HCGRID_ERR_INVALID_ARG, "the kernel cannot change while an accumulation is open");
     KernelParams& kp = c->kp;
@@ -187,6 +199,7 @@ int hcgrid_set_target_car(hcgrid_ctx* c, int32_t nx, int32_t ny, double lon0, do
     HCG_CUDA(c, cudaSetDevice(c->device));
     c->has_target = false;
     c->acc_nchan = 0;
+    ++c->config_gen;
     return build_target_car(c, nx, ny, lon0, lat0, dlon, dlat);
 }
 
@@ -198,6 +211,7 @@ int hcgrid_set_target_cells(hcgrid_ctx* c, int64_t ncell, const double* lon, con
     HCG_CUDA(c, cudaSetDevice(c->device));
     c->has_target = false;
     c->acc_nchan = 0;
+    ++c->config_gen;
     return build_target_cells(c, ncell, lon, lat, (cudaStream_t)stream);
 }
 
@@ -213,8 +227,56 @@ int hcgrid_grid(hcgrid_ctx* c, int64_t n, const double* lon, const double* lat, 
     cudaStream_t st = (cudaStream_t)stream;
     c->last_lon = lon; c->last_lat = lat; c->last_n = n; c->last_stream = st;
     c->ev_valid = false;
+    // A call that repeats the previous one (same arrays, sizes, options, target) is replayed as a CUDA graph: below
+    // ~1e6 samples the call is bound by the launch gaps of its 7-9 dependent kernels, not by their work.  The second
+    // identical call captures (on a stream of the context's own: nothing runs during capture, and the caller's stream
+    // may be the legacy default stream, which cannot capture); every later one is a single graph launch.
+    const bool graph_ok = !c->opt_profile && c->acc_nchan == 0 && n > 0 &&
+                          (c->opt_graph == 1 || (c->opt_graph < 0 && n <= kGraphMaxN));
+    const hcgrid_ctx::GraphKey key{n, lon, lat, values, weights, cube, wmap, counts, nchan, c->config_gen};
+    if (graph_ok && c->graph_valid && c->graph_key == key) {
+        HCG_CUDA(c, cudaGraphLaunch(c->graph_exec, st));
+        c->stats = c->graph_stats;
+        c->stats.n_kept = -1;
+        c->stat_hit = c->stat_pairs = false;
+        return HCGRID_OK;
+    }
     c->stats = hcgrid_stats{};
     c->stats.n_samples = n;
+    if (graph_ok && c->graph_seen_valid && c->graph_seen == key) {
+        if (!c->st_cap) HCG_CUDA(c, cudaStreamCreateWithFlags(&c->st_cap, cudaStreamNonBlocking));
+        if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+        c->graph_valid = false;
+        cudaGraph_t graph = nullptr;
+        HCG_CUDA(c, cudaStreamBeginCapture(c->st_cap, cudaStreamCaptureModeThreadLocal));
+        int rc = run_preorder(c, n, lon, lat, values, nchan, weights, c->st_cap);
+        if (rc == HCGRID_OK) rc = run_convolve(c, n, values, nchan, weights != nullptr, cube, wmap, counts, c->st_cap);
+        const cudaError_t e = cudaStreamEndCapture(c->st_cap, &graph);
+        if (rc == HCGRID_OK && e == cudaSuccess && graph != nullptr &&
+            cudaGraphInstantiate(&c->graph_exec, graph, 0) == cudaSuccess) {
+            cudaGraphDestroy(graph);
+            c->graph_key = key;
+            c->graph_valid = true;
+            c->graph_stats = c->stats;
+            c->graph_stats.graph = 1;
+            c->stats = c->graph_stats;
+            HCG_CUDA(c, cudaGraphLaunch(c->graph_exec, st));
+            c->stats.n_kept = -1;
+            c->stat_hit = c->stat_pairs = false;
+            return HCGRID_OK;
+        }
+        // capture refused (a call inside that may not be captured): run eagerly, do not try again for this key
+        if (graph) cudaGraphDestroy(graph);
+        if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+        cudaGetLastError();
+        c->graph_seen_valid = false;
+        c->err.clear();
+        c->stats = hcgrid_stats{};
+        c->stats.n_samples = n;
+    } else {
+        c->graph_seen = key;
+        c->graph_seen_valid = graph_ok;
+    }
     int rc = run_preorder(c, n, lon, lat, values, nchan, weights, st);
     if (rc != HCGRID_OK) return rc;
     rc = run_convolve(c, n, values, nchan, weights != nullptr, cube, wmap, counts, st);

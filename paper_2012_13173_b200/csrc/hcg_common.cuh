@@ -95,6 +95,7 @@ struct Region {            // what of the sphere the target can reach (host + de
     double sx32, sy32;     // fixed-point units per radian (lon, lat): 2^32 over a span >= wx / wy (target.cu)
 };
 
+constexpr int64_t kGraphMaxN = 1 << 21;   // auto: calls of up to this many samples are replayed as a CUDA graph
 constexpr double kF32RadiusMax = 0.004;   // rad: largest support radius of the fp32 pair arithmetic (target.cu)
 
 struct KernelParams {      // per-context constants of the pair arithmetic
@@ -174,6 +175,23 @@ struct hcgrid_ctx {
     cudaStream_t st_copy = nullptr, st_comp = nullptr;   // hcgrid_grid_host pipeline (created on first use)
     cudaEvent_t ev_chunk[16] = {};
     int opt_host_chunks = 0;
+    int opt_cells_as_grid = 1;           // HCGRID_OPT_CELLS_AS_GRID
+    // Replay of repeated small calls (HCGRID_OPT_GRAPH): the kernels of one hcgrid_grid call as an instantiated CUDA
+    // graph, keyed by everything a launch depends on; config_gen counts option / kernel / target changes.
+    int opt_graph = -1;                  // -1 auto (inputs up to kGraphMaxN samples), 0 off, 1 on for any size
+    uint64_t config_gen = 0;
+    struct GraphKey {
+        int64_t n; const void *lon, *lat, *values, *weights, *cube, *wmap, *counts; int32_t nchan; uint64_t gen;
+        bool operator==(const GraphKey& o) const {
+            return n == o.n && lon == o.lon && lat == o.lat && values == o.values && weights == o.weights && cube == o.cube &&
+                   wmap == o.wmap && counts == o.counts && nchan == o.nchan && gen == o.gen;
+        }
+    };
+    GraphKey graph_key{}, graph_seen{};  // key of the instantiated graph / of the last eager call
+    bool graph_valid = false, graph_seen_valid = false;
+    cudaGraphExec_t graph_exec = nullptr;
+    hcgrid_stats graph_stats{};
+    cudaStream_t st_cap = nullptr;       // capture happens here; the graph is launched into the caller's stream
     cudaEvent_t ev[8] = {};
     bool ev_valid = false;
     bool stat_hit = false, stat_pairs = false;   // d_stat[0] / d_stat[1] hold n_hit / n_pairs_tested of the last call

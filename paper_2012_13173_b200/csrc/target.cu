@@ -253,11 +253,72 @@ int build_target_car(hcgrid_ctx* c, int nx, int ny, double lon0, double lat0, do
     return finish_target(c, hs, nx, std::min(a, b), std::max(a, b));
 }
 
+// Step of an arithmetic progression v[0], v[stride], ..., v[(n - 1) stride] in the plate-carree convention
+// v0 + k * d (one rounding per operation): tried are the first difference, the mean difference and their
+// neighbours within two units in the last place.  tol = 0: every term must match bit for bit.
+static bool find_step(const double* v, int64_t n, int64_t stride, double tol, double& d_out) {
+    if (n < 2) return false;
+    const double v0 = v[0];
+    const double base[2] = {v[stride] - v0, (v[(n - 1) * stride] - v0) / (double)(n - 1)};
+    for (int b = 0; b < 2; ++b)
+        for (int k = -2; k <= 2; ++k) {
+            double d = base[b];
+            for (int s = 0; s < std::abs(k); ++s) d = std::nextafter(d, k > 0 ? HUGE_VAL : -HUGE_VAL);
+            if (d == 0.0 || !std::isfinite(d)) continue;
+            bool ok = true;
+            for (int64_t i = 0; i < n && ok; ++i) {
+                volatile double prod = (double)i * d;
+                volatile double x = v0 + prod;
+                ok = tol == 0.0 ? x == v[i * stride] : std::fabs(x - v[i * stride]) <= tol;
+            }
+            if (ok) { d_out = d; return true; }
+        }
+    return false;
+}
+
+// Per-cell targets that are a plate-carree grid listed row by row (what a WCS CAR header expands to) are recognised
+// and take the plate-carree path with its tile kernels.  fp64 mode: only if lon0 + ix * dlon, lat0 + iy * dlat
+// reproduce every given centre bit for bit (the results are then those of the general path on the same centres);
+// fp32 mode: to 1e-10 deg (1.7e-12 rad: far inside the 1e-9 rad of the count bar and 1e-7 of the fp32 tolerance).
+static bool detect_car(const std::vector<double>& hl, const std::vector<double>& hb, bool exact, int& nx, int& ny,
+                       double& dlon, double& dlat) {
+    const int64_t ncell = (int64_t)hl.size();
+    const double tol = exact ? 0.0 : 1e-10;
+    int64_t w = 1;
+    while (w < ncell && (exact ? hb[(size_t)w] == hb[0] : std::fabs(hb[(size_t)w] - hb[0]) <= tol)) ++w;
+    if (w < 2 || ncell % w != 0 || w > (1 << 30) || ncell / w > (1 << 30)) return false;
+    const int64_t h = ncell / w;
+    if (!find_step(hl.data(), w, 1, tol, dlon)) return false;
+    dlat = 1.0;                                               // a single row: any non-zero step
+    if (h > 1 && !find_step(hb.data(), h, w, tol, dlat)) return false;
+    if (std::fabs(dlon) * (double)(w - 1) >= 360.0) return false;
+    for (int64_t iy = 0; iy < h; ++iy) {
+        const double lat_row = hb[(size_t)(iy * w)];
+        for (int64_t ix = 0; ix < w; ++ix) {
+            const double l = hl[(size_t)(iy * w + ix)], b = hb[(size_t)(iy * w + ix)];
+            if (exact ? (l != hl[(size_t)ix] || b != lat_row)
+                      : (std::fabs(l - hl[(size_t)ix]) > tol || std::fabs(b - lat_row) > tol))
+                return false;
+        }
+    }
+    nx = (int)w; ny = (int)h;
+    return true;
+}
+
 int build_target_cells(hcgrid_ctx* c, int64_t ncell, const double* lon, const double* lat, cudaStream_t st) {
     std::vector<double> hl((size_t)ncell), hb((size_t)ncell);
     HCG_CUDA(c, cudaMemcpyAsync(hl.data(), lon, sizeof(double) * (size_t)ncell, cudaMemcpyDeviceToHost, st));
     HCG_CUDA(c, cudaMemcpyAsync(hb.data(), lat, sizeof(double) * (size_t)ncell, cudaMemcpyDeviceToHost, st));
     HCG_CUDA(c, cudaStreamSynchronize(st));
+    {
+        int nx = 0, ny = 0;
+        double dlon = 0.0, dlat = 0.0;
+        bool valid = true;
+        for (int64_t i = 0; i < ncell && valid; ++i)
+            valid = hb[(size_t)i] >= -90.0 && hb[(size_t)i] <= 90.0 && std::isfinite(hl[(size_t)i]);
+        if (valid && c->opt_cells_as_grid && detect_car(hl, hb, c->precision == HCGRID_F64, nx, ny, dlon, dlat))
+            return build_target_car(c, nx, ny, hl[0], hb[0], dlon, dlat);
+    }
     std::vector<HostStrip> hs((size_t)ncell);
     double sx = 0, sy = 0;
     for (int64_t i = 0; i < ncell; ++i) {

@@ -96,7 +96,9 @@ def test_tapered_sinc_negative_weight_cells_and_arbitrary_cells(oracle, precisio
     w = workloads.Workload("sparse", 1, 1.0, lon, lat, val, None, w0.sigma_deg, 3 * w0.sigma_deg, w0.nside, t)
     ref = _oracle(oracle, w, (oracle.TAPERED_SINC, A, B))
     assert np.sum(ref.weightmap < 0) > 0
-    cube, wmap, cnt, _ = _gpu(w, precision, (1, A, B), explicit_cells=True)
+    from paper_2012_13173_b200 import binding
+    cube, wmap, cnt, st = _gpu(w, precision, (1, A, B), explicit_cells=True, options={binding.OPT_CELLS_AS_GRID: 0})
+    assert st["kernel"] in (3, 5)                      # the per-cell path: general kernels
     r = _cmp(cube, wmap, cnt, ref, w, precision)
     assert r["negative_w_cells"] > 0
     neg = (ref.weightmap < 0) & (np.abs(ref.weightmap) >= 0.05 * ref.abswmap)

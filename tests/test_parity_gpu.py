@@ -244,9 +244,68 @@ def test_nside_invariance(oracle, nside):
 
 
 def test_explicit_cells_equal_car(oracle):
+    """A plate-carree grid handed over cell by cell is recognised and takes the plate-carree path (same kernel, same
+    bits); with the recognition off, or as soon as one centre is off the grid, the per-cell path runs."""
+    from paper_2012_13173_b200 import binding
     w, ref = mini(oracle, 2)
+    car = run_gpu(w, "f32")
     a = run_gpu(w, "f32", explicit_cells=True)
+    assert a[3]["kernel"] == car[3]["kernel"] == 6
+    for x, y in zip(a[:3], car[:3]):
+        assert np.array_equal(x, y, equal_nan=True)
     compare(a[0], a[1], a[2], ref, w.sigma_deg, w.radius_deg, TOL_F32)
+    b = run_gpu(w, "f32", {binding.OPT_CELLS_AS_GRID: 0}, explicit_cells=True)
+    assert b[3]["kernel"] in (1, 2, 3)
+    compare(b[0], b[1], b[2], ref, w.sigma_deg, w.radius_deg, TOL_F32)
+    # fp64 mode: recognised only because lon0 + ix * dlon reproduces every centre bit for bit -> same bits as the CAR call
+    car64 = run_gpu(w, "f64")
+    a64 = run_gpu(w, "f64", explicit_cells=True)
+    for x, y in zip(a64[:3], car64[:3]):
+        assert np.array_equal(x, y, equal_nan=True)
+    compare(a64[0], a64[1], a64[2], ref, w.sigma_deg, w.radius_deg, TOL_F64)
+
+
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+@pytest.mark.parametrize("case", ["one_cell_moved", "jitter_1e-12_deg", "rows_swapped", "single_row", "descending"])
+def test_explicit_cells_near_grids(oracle, case, precision):
+    """Cell lists that are almost, or in another sense, a plate-carree grid: whatever path is chosen, the result is the
+    oracle's on the centres as given."""
+    from paper_2012_13173_b200 import binding
+    w = workloads.make(1, 1.0)
+    t = w.target
+    cl, cb = t.cell_centers()
+    rng = np.random.default_rng(5)
+    grid_like = None                                     # None: either path may run
+    if case == "one_cell_moved":
+        cl = cl.copy(); cl[t.nx * 7 + 3] += 3e-4
+        grid_like = False
+    elif case == "jitter_1e-12_deg":
+        cl = cl + rng.uniform(-1e-12, 1e-12, cl.size)
+        cb = cb + np.repeat(rng.uniform(-1e-12, 1e-12, t.ny), t.nx)
+        grid_like = precision == "f32"                   # fp64 mode wants the centres bit for bit
+    elif case == "rows_swapped":
+        idx = np.arange(t.ncell).reshape(t.ny, t.nx)
+        idx[[2, 9]] = idx[[9, 2]]
+        cl, cb = cl[idx.ravel()], cb[idx.ravel()]
+        grid_like = False
+    elif case == "single_row":
+        cl, cb = cl[5 * t.nx:6 * t.nx], cb[5 * t.nx:6 * t.nx]
+        grid_like = True
+    elif case == "descending":
+        cl, cb = cl[::-1].copy(), cb[::-1].copy()        # a grid with negative steps: not bit-exact in general
+    ref = oracle.grid(w.sigma_deg, w.radius_deg, cl, cb, w.lon, w.lat, w.values, w.weights)
+    g = binding.HCGrid(w.sigma_deg, w.radius_deg, w.nside, precision=precision)
+    g.set_target_cells(_dev(cl), _dev(cb))
+    cube, wmap, cnt = g.grid(_dev(w.lon), _dev(w.lat), _dev(w.values))
+    torch.cuda.synchronize()
+    st = g.stats()
+    g.close()
+    if grid_like is not None and precision == "f32":
+        assert (st["kernel"] == 6) == grid_like
+    if grid_like is not None and precision == "f64" and not grid_like:
+        assert st["kernel"] == 5
+    compare(cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy(), ref, w.sigma_deg, w.radius_deg,
+            TOL_F32 if precision == "f32" else TOL_F64)
 
 
 def test_deterministic_bitwise():
