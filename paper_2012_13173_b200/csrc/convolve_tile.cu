@@ -31,7 +31,7 @@ template <int GX, int GY, int MODE, bool COUNTS, bool SPLIT, int KFN = 0>
 __global__ void __launch_bounds__(kMaxTileWarps * 32)
 conv1_tile_f32(const TileArgs a) {
     constexpr int NC = GX * GY;
-    __shared__ ulonglong2 s_tab[kMaxTileWarps][32];
+    __shared__ unsigned long long s_tab[kMaxTileWarps][32];
     __shared__ float s_pw[SPLIT ? kMaxTileWarps : 1][NC], s_ps[SPLIT ? kMaxTileWarps : 1][NC];   // partial sums of a split tile
     __shared__ int s_pc[SPLIT ? kMaxTileWarps : 1][NC];
     const int lane = threadIdx.x & 31;
@@ -90,7 +90,7 @@ conv1_tile_f32(const TileArgs a) {
     const float fxw = (float)(a.du >= 0.0 ? ix0 : ix0 + ncols - 1);   // westmost / eastmost column of the tile
     const float fxe = (float)(a.du >= 0.0 ? ix0 + ncols - 1 : ix0);
     const Rec32* __restrict__ rec = a.rec;
-    ulonglong2* tab = s_tab[wib];
+    unsigned long long* tab = s_tab[wib];
 
     for (int rb = rmin; rb <= rmax; rb += 32) {
         // ---- steps (ii)+(iii): lane k <-> ring rb + k
@@ -126,9 +126,8 @@ conv1_tile_f32(const TileArgs a) {
         }
         const int total = __shfl_sync(0xffffffffu, incl, 31);
         __syncwarp();                                   // previous pass done with the table
-        // (end of ring k in the stream, address of the record that would have stream index 0)
-        tab[lane] = make_ulonglong2((unsigned long long)(unsigned)incl,
-                                    (unsigned long long)(uintptr_t)(rec + ((long long)sa - (incl - sn))));
+        // (end of ring k in the stream, index of the record that would have stream index 0)
+        tab[lane] = (unsigned long long)(unsigned)incl | ((unsigned long long)(unsigned)(sa - (incl - sn)) << 32);
         __syncwarp();
         if (total == 0) continue;
 
@@ -139,21 +138,20 @@ conv1_tile_f32(const TileArgs a) {
         const int nfull = total >> 5;
         const int stride = 32 * S;
         uint32_t tp = smem_addr(tab);                   // ring cursor: shared address of entry k
-        unsigned long long end, base;
-        lds_entry(tp, end, base);
+        unsigned long long eb = lds_entry8(tp);
         int i = part * 32 + lane;
-        stream_seek(min(i, last), tp, end, base);
-        uint4 ra = ldg_rec(base, min(i, last));
+        stream_seek8(min(i, last), tp, eb);
+        uint4 ra = ldg_rec8(rec, eb, min(i, last));
         int i1 = i + stride;
-        stream_seek(min(i1, last), tp, end, base);
-        uint4 rn = ldg_rec(base, min(i1, last));
+        stream_seek8(min(i1, last), tp, eb);
+        uint4 rn = ldg_rec8(rec, eb, min(i1, last));
         tc.hm = tc.hmax;
 #pragma unroll 3
         for (int it = part; it < nfull; it += S) {
             const int i2 = i1 + stride;
             const int ii = min(i2, last);
-            stream_seek(ii, tp, end, base);
-            const uint4 rc = ldg_rec(base, ii);
+            stream_seek8(ii, tp, eb);
+            const uint4 rc = ldg_rec8(rec, eb, ii);
             tile_pairs<GX, GY, MODE, COUNTS, KFN>(ra, tc, W, S_, cnt);
             ra = rn; rn = rc;
             i = i1; i1 = i2;

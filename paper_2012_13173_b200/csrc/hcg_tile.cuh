@@ -174,6 +174,30 @@ __device__ __forceinline__ uint4 ldg_rec(unsigned long long base, int i) {
     return __ldg((const uint4*)(uintptr_t)(base + (unsigned long long)(unsigned)i * 16ull));
 }
 
+// The same cursor with 8-byte table entries (the tile kernel): low word = end of ring k in the stream, high word =
+// record index of the record that would have stream index 0 (may be negative).  One 64-bit load lands in the
+// register pair that holds the entry -- no copies -- and the record address is rec + (base + i).
+__device__ __forceinline__ unsigned long long lds_entry8(uint32_t tp) {
+    unsigned long long eb;
+    asm volatile("ld.shared.u64 %0, [%1];" : "=l"(eb) : "r"(tp));
+    return eb;
+}
+__device__ __forceinline__ void stream_seek8(int i, uint32_t& tp, unsigned long long& eb) {
+    asm volatile("{\n\t.reg .pred p;\n\t.reg .b32 e, b;\n\t"
+                 "mov.b64 {e, b}, %0;\n\t"
+                 "setp.ge.s32 p, %2, e;\n\t"
+                 "@p add.u32 %1, %1, 8;\n\t"
+                 "@p ld.shared.u64 %0, [%1];\n\t}"
+                 : "+l"(eb), "+r"(tp) : "r"(i));
+    while (i >= (int)(uint32_t)eb) {
+        tp += 8;
+        eb = lds_entry8(tp);
+    }
+}
+__device__ __forceinline__ uint4 ldg_rec8(const Rec32* __restrict__ rec, unsigned long long eb, int i) {
+    return __ldg((const uint4*)rec + ((int)(eb >> 32) + i));
+}
+
 constexpr int ilog2(int n) { return n <= 1 ? 0 : 1 + ilog2(n / 2); }
 
 // Host side: the fields of TileArgs that depend only on the context (not on the tile shape
