@@ -41,7 +41,7 @@ UNIT = "cell-channels/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` captures (profiles/): (config, stats kernel id) -> (bytes, source)
 NCU_TRAFFIC = {
-    (3, 6): (191985408 + 12509952, "profiles/r01e_conv1_tile_ncu_full.md"),
+    (3, 6): (191993856 + 12059648, "profiles/r02_conv1_tile_ncu_full.md"),
     (4, 7): (3714980000 + 98979072, "profiles/r01c_conv_mc_ncu_full.md"),
     (4, 8): (1368034000 + 81781760, "profiles/r02_conv_mc_tc_ncu_full.md"),
 }
