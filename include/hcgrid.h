@@ -228,6 +228,23 @@ int hcgrid_host_ring_info(int64_t nside, int32_t iring, int64_t* first_pixel, in
  * Synchronises the device. */
 int hcgrid_measure_peaks(int device, double* fp32_inst_per_s, double* mufu_per_s);
 
+/* The one entry point that ALLOCATES NOTHING (no cudaMalloc / cudaFree / allocating library routine), for callers
+ * that cannot allocate: code under CUDA-graph capture, tight serving loops, harnesses that forbid it.  Every other
+ * call of this library may grow a context-owned device buffer.  From the count output of hcgrid_grid (PAPER.md:59:
+ * the samples with d <= R of every cell) it forms the figures the throughput metric is quoted in:
+ *   out[0] = sum of counts[0 .. ncell)           -- pairs (cell, sample) with d <= R ("kernel evaluations", n_hit)
+ *   out[1] = number of cells with counts[i] > 0  -- cells the samples reach
+ * counts [ncell] int32 and out [2] uint64 are DEVICE pointers on the CURRENT device, owned by the caller;
+ * asynchronous on `stream`; no context needed.  Its scratch (per-block partial sums and a ticket) is a fixed
+ * 16.25 KB device array inside the library, held by every GPU that loads it until the process exits; hence
+ *   - ncell <= hcgrid_static_max_cells() = 2^30, more is refused with HCGRID_ERR_INVALID_ARG;
+ *   - ALL calls on one device share the array: calls that overlap on the GPU (two streams, two host threads)
+ *     race and give wrong sums -- serialise them.  Calls one after the other on a stream are fine (what must start
+ *     at zero is cleared at the start of every call).
+ * Same sums as hcgrid_stats.n_hit (integers, fixed order).  Errors: status + hcgrid_last_error(NULL). */
+int hcgrid_count_hits_static(const int32_t* counts, int64_t ncell, uint64_t* out, void* stream);
+int64_t hcgrid_static_max_cells(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -31,7 +31,7 @@ EXPORTS = [
     "hcgrid_get_stats", "hcgrid_last_error", "hcgrid_debug_preorder",
     "hcgrid_debug_ang2pix_ring", "hcgrid_host_ang2pix_ring", "hcgrid_host_ring_info",
     "hcgrid_measure_peaks", "hcgrid_accumulate", "hcgrid_finalize", "hcgrid_accumulated_batches",
-    "hcgrid_set_kernel",
+    "hcgrid_set_kernel", "hcgrid_count_hits_static", "hcgrid_static_max_cells",
 ]
 KERNEL_GAUSS, KERNEL_TAPERED_SINC, KERNEL_ELLIPTICAL_GAUSS = 0, 1, 2          # hcgrid_set_kernel types
 
@@ -94,8 +94,11 @@ def load_library():
     lib.hcgrid_host_ring_info.argtypes = [i64, i32, ctypes.POINTER(i64), ctypes.POINTER(i32),
                                           ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
     lib.hcgrid_measure_peaks.argtypes = [ctypes.c_int, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
+    lib.hcgrid_count_hits_static.argtypes = [vp, i64, vp, vp]
+    lib.hcgrid_static_max_cells.argtypes = []
+    lib.hcgrid_static_max_cells.restype = i64
     for name in EXPORTS:
-        if name not in ("hcgrid_ncell", "hcgrid_last_error", "hcgrid_accumulated_batches"):
+        if name not in ("hcgrid_ncell", "hcgrid_last_error", "hcgrid_accumulated_batches", "hcgrid_static_max_cells"):
             getattr(lib, name).restype = ctypes.c_int
     _lib = lib
     return lib
@@ -137,6 +140,31 @@ def measure_peaks(device: int = 0):
     if rc != 0:
         raise HCGridError(rc, lib.hcgrid_last_error(None).decode())
     return a.value, b.value
+
+
+def static_max_cells() -> int:
+    return int(load_library().hcgrid_static_max_cells())
+
+
+def count_hits_static(counts, out=None, ncell: Optional[int] = None):
+    """hcgrid_count_hits_static: (sum of counts, cells with counts > 0) of an int32 CUDA tensor into `out`, a uint64-sized
+    (torch.int64) CUDA tensor of 2 entries -- allocated here only if the caller passes none.  The library call itself
+    allocates nothing; asynchronous on torch's current stream.  Calls that overlap on one GPU race (shared scratch)."""
+    import torch
+    lib = load_library()
+    if not (counts.is_cuda and counts.dtype == torch.int32 and counts.is_contiguous()):
+        raise TypeError("counts must be a contiguous CUDA int32 tensor")
+    if out is None:
+        out = torch.empty(2, dtype=torch.int64, device=counts.device)
+    if not (out.is_cuda and out.dtype == torch.int64 and out.numel() >= 2 and out.is_contiguous()):
+        raise TypeError("out must be a contiguous CUDA int64 tensor of 2 entries")
+    n = counts.numel() if ncell is None else int(ncell)
+    with torch.cuda.device(counts.device):
+        st = torch.cuda.current_stream().cuda_stream
+        rc = lib.hcgrid_count_hits_static(counts.data_ptr(), n, out.data_ptr(), st)
+    if rc != 0:
+        raise HCGridError(rc, lib.hcgrid_last_error(None).decode())
+    return out
 
 
 def ang2pix_ring(nside: int, lon_deg, lat_deg):

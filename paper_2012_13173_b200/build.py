@@ -14,7 +14,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libhcgrid.so")
-SOURCES = ["api.cu", "target.cu", "preorder.cu", "convolve.cu", "convolve_tile.cu", "convolve_mc.cu", "convolve_mc_tc.cu", "convolve_gen.cu", "accumulate.cu", "debug.cu"]
+SOURCES = ["api.cu", "target.cu", "preorder.cu", "convolve.cu", "convolve_tile.cu", "convolve_mc.cu", "convolve_mc_tc.cu", "convolve_gen.cu", "accumulate.cu", "debug.cu", "no_alloc.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 
