@@ -542,11 +542,14 @@ conv_mc_tc_f32(const McTcArgs m) {
             const int slot = k % kTcNS;
             const uint32_t sb = s_base + (uint32_t)slot * kStageBytes + kOffBraw;
             if (on) {
-#pragma unroll
-                for (int i0 = 0; i0 < NU; i0 += 4) {
-                    uint4 v[4];
+                // two register buffers of 4 units take turns: the loads of one batch are in flight while the other is
+                // split and stored (the shared-memory wrappers are ordered among themselves, so the overlap has to be
+                // spelled out)
+                auto load4 = [&](uint4 (&v)[4], int i0) {
 #pragma unroll
                     for (int j = 0; j < 4; ++j) v[j] = lds_u4(sb + unit_off(i0 + j));
+                };
+                auto split4 = [&](uint4 (&v)[4], int i0) {
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {
                         uint4 l;
@@ -556,6 +559,15 @@ conv_mc_tc_f32(const McTcArgs m) {
                         l.w = __float_as_uint(__uint_as_float(v[j].w) - __uint_as_float(v[j].w & 0xffffe000u));
                         sts_u4(sb + (kOffBlo - kOffBraw) + unit_off(i0 + j), l);
                     }
+                };
+                uint4 va[4], vb[4];
+                load4(va, 0);
+#pragma unroll
+                for (int i0 = 0; i0 < NU; i0 += 8) {
+                    load4(vb, i0 + 4);
+                    split4(va, i0);
+                    if (i0 + 8 < NU) load4(va, i0 + 8);
+                    split4(vb, i0 + 4);
                 }
             }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -709,24 +721,41 @@ conv_mc_tc_f32(const McTcArgs m) {
         if (__any_sync(0xffffffffu, chk != 0.0f) && lane == 0) atomicOr(s_bad, 1);
         bar_compute();
         const float wtot = s_w[cell] + s_w[128 + cell];
-        if (cell_ok) {
+        // what the sums are multiplied by: 1 / W (one division per cell; a product differs from the quotient by at most
+        // 1.5 ulp), NaN for a cell no sample reaches, 1 for un-normalised sums
+        const float scale = a.raw ? 1.0f : (wtot > 0.0f ? 1.0f / wtot : __int_as_float(0x7fc00000));
+        if (cell_ok && g == 0 && blockIdx.y == 0) {
             const int64_t gc = (int64_t)(row0 + ciy) * a.nx + ix0 + cix;
-            if (g == 0 && blockIdx.y == 0) {
-                a.wmap[gc] = wtot;
-                if (COUNTS) a.counts[gc] = s_c[cell] + s_c[128 + cell];
-            }
-            float* o = a.cube + (size_t)gc * m.nchan + ch0 + g * 128;
-            const float nan = __int_as_float(0x7fc00000);
-            const bool filled = wtot > 0.0f;
+            a.wmap[gc] = wtot;
+            if (COUNTS) a.counts[gc] = s_c[cell] + s_c[128 + cell];
+        }
+        // The sums go out through shared memory (the stage buffers are idle by now: every MMA has completed and the row
+        // warps have left): a thread holds 128 channels of ONE cell, so direct stores would touch 32 cells' rows per
+        // instruction; transposed, a warp writes 512 contiguous bytes of one cell per instruction.
+        constexpr uint32_t kPitch = 1024 + 16;                       // bytes per cell row (+ 16: conflict-free 16-byte columns)
+        static_assert(128 * kPitch <= (uint32_t)kOffFifoX, "epilogue staging");
+        {
+            const uint32_t so = s_base + (uint32_t)cell * kPitch + (uint32_t)g * 512u;
 #pragma unroll
-            for (int j = 0; j < 128; j += 4) {
-                if (g * 128 + j < nch) {
-                    float4 f;
-                    f.x = a.raw ? acc[j] : (filled ? acc[j] / wtot : nan);
-                    f.y = a.raw ? acc[j + 1] : (filled ? acc[j + 1] / wtot : nan);
-                    f.z = a.raw ? acc[j + 2] : (filled ? acc[j + 2] / wtot : nan);
-                    f.w = a.raw ? acc[j + 3] : (filled ? acc[j + 3] / wtot : nan);
-                    *(float4*)(o + j) = f;
+            for (int j = 0; j < 128; j += 4)
+                sts_u4(so + 4u * j, make_uint4(__float_as_uint(acc[j] * scale), __float_as_uint(acc[j + 1] * scale),
+                                               __float_as_uint(acc[j + 2] * scale), __float_as_uint(acc[j + 3] * scale)));
+        }
+        bar_compute();
+        {
+            const int nu = nch >> 2;                                  // 16-byte units per cell (<= 64)
+            for (int cl = warp; cl < 128; cl += kTcCW) {              // cell 32 q' + l' of the tile
+                const int ex = 8 * ((cl >> 5) & 1) + (cl & 7), ey = 4 * (cl >> 6) + ((cl & 31) >> 3);
+                if (ex >= ncols || ey >= nrows) continue;             // warp-uniform
+                float* o = a.cube + ((size_t)(row0 + ey) * a.nx + ix0 + ex) * m.nchan + ch0;
+                const uint32_t si = s_base + (uint32_t)cl * kPitch;
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int u = lane + 32 * h;
+                    if (u < nu) {
+                        const uint4 v = lds_u4(si + 16u * u);
+                        *(uint4*)(o + 4 * u) = v;
+                    }
                 }
             }
         }
