@@ -43,7 +43,7 @@ UNIT = "cell-channels/s"
 NCU_TRAFFIC = {
     (3, 6): (191993856 + 12059648, "profiles/r02_conv1_tile_ncu_full.md"),
     (4, 7): (3714980000 + 98979072, "profiles/r01c_conv_mc_ncu_full.md"),
-    (4, 8): (1368034000 + 81781760, "profiles/r02_conv_mc_tc_ncu_full.md"),
+    (4, 8): (1365308000 + 83858944, "profiles/r02_conv_mc_tc_ncu_full.md"),
 }
 WORKLOAD_NAMES = {1: "config1_tiny_20k", 2: "config2_drift_scan_1.25M", 3: "config3_dense_10M",
                   4: "config4_spectral_cube_1M_x256", 5: "config5_polar_20M"}
@@ -245,11 +245,14 @@ def run_product(args):
     g.set_option(binding.OPT_PROFILE, 1)
     stage = {k: [] for k in ("us_pixelise", "us_sort", "us_tables", "us_pack", "us_convolve", "us_total")}
     step(); torch.cuda.synchronize()
-    for _ in range(args.steps):
+    # the stage events are read (a host synchronisation) after every fourth call only, so that the calls that are
+    # measured run back to back like those of the timed region: after an idle gap the same kernels run 5-7 % slower
+    for i in range(args.steps):
         step()
-        s = g.stats()
-        for k in stage:
-            stage[k].append(s[k])
+        if i % 4 == 3 or args.steps < 4:
+            s = g.stats()
+            for k in stage:
+                stage[k].append(s[k])
     st = g.stats()
     # the same call with the count output (untimed for `value`; its convolution time is reported)
     us_conv_counts = []

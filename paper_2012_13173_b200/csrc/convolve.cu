@@ -412,7 +412,7 @@ int run_convolve(hcgrid_ctx* c, int64_t n, const float* values, int nchan, bool 
                     "multiple of 32");
     if (tc_ok && (c->opt_kernel == 7 || (c->opt_kernel == 0 && nchan >= 64))) {
         const size_t nd = (size_t)mc_tc_tiles(c) * (size_t)((nchan + 255) / 256);
-        HCG_CUDA(c, c->d_dirty.ensure(nd * 4));
+        HCG_CUDA(c, c->d_dirty.ensure((nd + (size_t)mc_tc_tiles(c) + 1) * 4));   // flags, list of flagged tiles, their count
         rc = launch_conv_mc_tc(c, values, nchan, (float*)cube, (float*)wmap, counts, c->d_dirty.as<int32_t>(), st);
         // tiles that met a non-finite value (0 * inf would poison all their cells) are redone cell by cell
         if (rc == HCGRID_OK) {
@@ -420,7 +420,7 @@ int run_convolve(hcgrid_ctx* c, int64_t n, const float* values, int nchan, bool 
             rc = launch_conv_general(c, a, false, false, st, c->d_dirty.as<int32_t>());
         }
         c->stats.kernel = 8;
-        if (rc == HCGRID_OK) c->stats.gpu_launches += 1;
+        if (rc == HCGRID_OK) c->stats.gpu_launches += 2;   // the list of flagged tiles and the pass over it
     } else if (mc_ok && (c->opt_kernel == 0 || c->opt_kernel == 6)) {
         rc = launch_conv_mc(c, values, nchan, (float*)cube, (float*)wmap, counts, st);
         c->stats.kernel = 7;

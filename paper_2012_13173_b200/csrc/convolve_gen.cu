@@ -11,6 +11,8 @@
 //
 // fp64 pair arithmetic follows the definition with no shortcut: differences formed in
 // degrees first, haversine, d = 2 asin(sqrt(hav)), w = exp(-d^2/(2 sigma^2)).
+#include <algorithm>
+
 #include "hcg_conv.cuh"
 
 namespace hcg {
@@ -129,20 +131,10 @@ __device__ __forceinline__ bool pair32_elliptical(const Rec32& r, const TaskCons
 
 // KFN: kernel function (hcgrid_set_kernel), 0 Gaussian, 1 tapered sinc, 2 elliptical Gaussian -- a template parameter so
 // that the Gaussian instantiations carry none of the other's code.
+// one cell (strip s, column ix) by one warp
 template <bool PAIR64, typename AccT, bool VEC4, int KFN>
-__global__ void __launch_bounds__(256)
-conv_general(const ConvArgs a) {
-    const int lane = threadIdx.x & 31;
-    const int64_t task = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (task >= a.ntasks) return;
-    const int s = (int)(task / a.strip_cells);
-    const int ix = (int)(task % a.strip_cells);
-    if (a.dirty) {                                              // warp-uniform
-        const int t16 = (s >> 3) * a.dirty_tiles_x + (ix >> 4);
-        int any = 0;
-        for (int b = 0; b < a.dirty_nblk; ++b) any |= __ldg(a.dirty + (size_t)b * a.dirty_ntiles + t16);
-        if (!any) return;
-    }
+__device__ __forceinline__ void conv_general_cell(const ConvArgs& a, const int s, const int ix, const int lane) {
+    const int64_t task = (int64_t)s * a.strip_cells + ix;
     const Strip st = a.strips[s];
     const int nchan = a.nchan;
     const float* __restrict__ values = a.values;
@@ -271,22 +263,65 @@ conv_general(const ConvArgs a) {
     }
 }
 
+template <bool PAIR64, typename AccT, bool VEC4, int KFN>
+__global__ void __launch_bounds__(256)
+conv_general(const ConvArgs a) {
+    const int64_t task = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (task >= a.ntasks) return;
+    conv_general_cell<PAIR64, AccT, VEC4, KFN>(a, (int)(task / a.strip_cells), (int)(task % a.strip_cells), threadIdx.x & 31);
+}
+
+// The fix-up pass after the tensor-core cube kernel: only the cells of the 16 x 8-cell tiles on the list (tiles that met a
+// non-finite value; usually none, and then every warp leaves at once), a warp at a time.
+template <bool PAIR64, typename AccT, bool VEC4, int KFN>
+__global__ void __launch_bounds__(256)
+conv_general_listed(const ConvArgs a) {
+    const int64_t ncells = (int64_t)__ldg(a.dirty_count) * 128;
+    const int64_t nw = (int64_t)gridDim.x * (blockDim.x >> 5);
+    for (int64_t wt = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); wt < ncells; wt += nw) {
+        const int t16 = __ldg(a.dirty_list + (wt >> 7)), cl = (int)(wt & 127);
+        const int s = (t16 / a.dirty_tiles_x) * 8 + (cl >> 4), ix = (t16 % a.dirty_tiles_x) * 16 + (cl & 15);
+        if (s < a.nstrip && ix < a.strip_cells) conv_general_cell<PAIR64, AccT, VEC4, KFN>(a, s, ix, threadIdx.x & 31);
+    }
+}
+
+// list of the tiles flagged in any channel block of dirty[nblk][ntiles]; *count must be zero on entry
+__global__ void __launch_bounds__(256)
+dirty_list_kernel(const int32_t* __restrict__ dirty, int nblk, int ntiles, int32_t* __restrict__ list, int32_t* __restrict__ count) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= ntiles) return;
+    int any = 0;
+    for (int b = 0; b < nblk; ++b) any |= __ldg(dirty + (size_t)b * ntiles + t);
+    if (any) list[atomicAdd(count, 1)] = t;             // order irrelevant: every cell is computed on its own
+}
+
 int launch_conv_general(hcgrid_ctx* c, const ConvArgs& a0, bool pair_f64, bool out_double, cudaStream_t st,
                         const int32_t* dirty) {
     ConvArgs a = a0;
-    a.dirty = dirty;
-    a.dirty_tiles_x = (c->strip_cells + 15) / 16;
-    a.dirty_ntiles = mc_tc_tiles(c);
-    a.dirty_nblk = (a.nchan + 255) / 256;
     a.ntasks = c->ncell;
     a.tasks_per_strip = a.strip_cells;
+    a.nstrip = c->nstrip;
     const bool vec4 = (a.nchan % 4 == 0) && ((uintptr_t)a.values % 16 == 0);
     const int threads = 256;
-    const unsigned blocks = (unsigned)((a.ntasks + 7) / 8);
+    unsigned blocks = (unsigned)((a.ntasks + 7) / 8);
     if (blocks == 0) return HCGRID_OK;
+    if (dirty) {
+        // dirty [nblk][ntiles] is followed by the list of flagged tiles [ntiles] and their count (convolve.cu sizes it)
+        const int ntiles = mc_tc_tiles(c), nblk = (a.nchan + 255) / 256;
+        a.dirty_tiles_x = (c->strip_cells + 15) / 16;
+        int32_t* list = const_cast<int32_t*>(dirty) + (size_t)nblk * ntiles;
+        int32_t* count = list + ntiles;
+        a.dirty_list = list;
+        a.dirty_count = count;
+        HCG_CUDA(c, cudaMemsetAsync(count, 0, 4, st));
+        dirty_list_kernel<<<(unsigned)((ntiles + 255) / 256), 256, 0, st>>>(dirty, nblk, ntiles, list, count);
+        HCG_CUDA(c, cudaGetLastError());
+        blocks = std::min<unsigned>(blocks, (unsigned)(8 * c->num_sms));
+    }
 #define HCG_LAUNCH(P, T, V)                                                        \
     do {                                                                           \
-        if (a.kp.ktype == 0) conv_general<P, T, V, 0><<<blocks, threads, 0, st>>>(a); \
+        if (dirty) conv_general_listed<P, T, V, 0><<<blocks, threads, 0, st>>>(a);  \
+        else if (a.kp.ktype == 0) conv_general<P, T, V, 0><<<blocks, threads, 0, st>>>(a); \
         else if (a.kp.ktype == 1) conv_general<P, T, V, 1><<<blocks, threads, 0, st>>>(a); \
         else conv_general<P, T, V, 2><<<blocks, threads, 0, st>>>(a);              \
     } while (0)

@@ -26,9 +26,10 @@ struct ConvArgs {
     float qx, qy;               // radians per fixed-point unit
     double sx;                  // fixed-point units per radian (lon)
     // fix-up pass of the general kernel after the tensor-core cube kernel (convolve_mc_tc.cu): only the cells of
-    // the 16 x 8-cell tiles flagged in dirty[blk * dirty_ntiles + tile] are recomputed (nullptr: every cell)
-    const int32_t* dirty;
-    int32_t dirty_tiles_x, dirty_ntiles, dirty_nblk;
+    // the dirty_count[0] tiles of 16 x 8 cells listed in dirty_list are recomputed (conv_general_listed)
+    const int32_t* dirty_list;
+    const int32_t* dirty_count;
+    int32_t dirty_tiles_x, nstrip;
 };
 
 __device__ __forceinline__ float ex2_approx(float x) {
