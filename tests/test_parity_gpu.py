@@ -399,6 +399,27 @@ def test_single_cell_single_sample():
         g.close()
 
 
+def test_nside_limits(oracle):
+    """nside is a power of two up to 16384 (12 nside^2 <= 2^32: the pixel index fits the sort key); the largest one
+    grids like any other (results do not depend on nside: reading c11)."""
+    from paper_2012_13173_b200 import binding
+    w, ref = mini(oracle, 1)
+    a = run_gpu(w, "f32", nside=16384)
+    compare(a[0], a[1], a[2], ref, w.sigma_deg, w.radius_deg, TOL_F32)
+    assert a[3]["n_kept"] > 0
+    d = run_gpu(w, "f64", nside=16384)
+    compare(d[0], d[1], d[2], ref, w.sigma_deg, w.radius_deg, TOL_F64)
+    for bad in (32768, 3000, 0):
+        with pytest.raises(binding.HCGridError):
+            binding.HCGrid(w.sigma_deg, w.radius_deg, bad)
+    # device and host pixelisation agree at the largest nside (indices up to 3.2e9: beyond int32)
+    rng = np.random.default_rng(16384)
+    lon, lat = rng.uniform(0, 360, 4000), np.rad2deg(np.arcsin(rng.uniform(-1, 1, 4000)))
+    dev = binding.ang2pix_ring(16384, _dev(lon), _dev(lat)).cpu().numpy()
+    host = binding.host_ang2pix_ring(16384, lon, lat)
+    assert np.array_equal(dev, host) and host.max() > 2 ** 31 and host.max() < 12 * 16384 ** 2
+
+
 def test_error_statuses():
     from paper_2012_13173_b200 import binding
     with pytest.raises(binding.HCGridError):
