@@ -153,6 +153,13 @@ int hcgrid_set_target_car(hcgrid_ctx* ctx, int32_t nx, int32_t ny, double lon0_d
 int hcgrid_set_target_cells(hcgrid_ctx* ctx, int64_t ncell, const double* lon_deg,
                             const double* lat_deg, void* stream);
 
+/* Lookup-bin refinement: on a plate-carree target with automatic HCGRID_OPT_SUBPIX_BITS, a call that brings more than
+ * 10 samples per lookup bin rebuilds the target's tables with finer bins (towards 4 samples per bin, at most 2^6 bins
+ * per HEALPix pixel) when that brings the density to 10 per bin or less: the counting pre-order then applies and the
+ * search windows tighten.  That call
+ * synchronises `stream` and the device once; later calls keep the finer tables until a new target is set.  Results
+ * do not depend on the bin size beyond the order of the additions (reading c11). */
+
 /* Grid n samples onto the target.
  *   lon_deg, lat_deg [n] double; values [n][nchan] float; weights [n] float or NULL.
  *   datacube [ncell][nchan], weightmap [ncell]: float (F32) or double (F64).

@@ -200,6 +200,7 @@ int hcgrid_set_target_car(hcgrid_ctx* c, int32_t nx, int32_t ny, double lon0, do
     c->has_target = false;
     c->acc_nchan = 0;
     ++c->config_gen;
+    c->subpix_refined = -1000;
     return build_target_car(c, nx, ny, lon0, lat0, dlon, dlat);
 }
 
@@ -212,6 +213,7 @@ int hcgrid_set_target_cells(hcgrid_ctx* c, int64_t ncell, const double* lon, con
     c->has_target = false;
     c->acc_nchan = 0;
     ++c->config_gen;
+    c->subpix_refined = -1000;
     return build_target_cells(c, ncell, lon, lat, (cudaStream_t)stream);
 }
 
@@ -225,6 +227,12 @@ int hcgrid_grid(hcgrid_ctx* c, int64_t n, const double* lon, const double* lat, 
     if (!cube || !wmap) return fail(c, HCGRID_ERR_INVALID_ARG, "datacube / weightmap is NULL");
     HCG_CUDA(c, cudaSetDevice(c->device));
     cudaStream_t st = (cudaStream_t)stream;
+    if (c->acc_nchan == 0) {                                  // not in the middle of a running accumulation
+        bool rebuilt = false;
+        const int rcr = refine_target_for_density(c, n, st, &rebuilt);
+        if (rcr != HCGRID_OK) return rcr;
+        if (rebuilt) ++c->config_gen;
+    }
     c->last_lon = lon; c->last_lat = lat; c->last_n = n; c->last_stream = st;
     c->ev_valid = false;
     // A call that repeats the previous one (same arrays, sizes, options, target) is replayed as a CUDA graph: below

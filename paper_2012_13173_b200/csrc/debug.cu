@@ -59,7 +59,7 @@ extern "C" {
 
 int hcgrid_debug_ang2pix_ring(int64_t nside, int64_t n, const double* lon, const double* lat, int64_t* pix,
                               void* stream) {
-    if (nside < 1 || nside > 8192 || (nside & (nside - 1)) || n < 0 || (n > 0 && (!lon || !lat || !pix)))
+    if (nside < 1 || nside > 16384 || (nside & (nside - 1)) || n < 0 || (n > 0 && (!lon || !lat || !pix)))
         return fail(nullptr, HCGRID_ERR_INVALID_ARG, "hcgrid_debug_ang2pix_ring: bad arguments");
     if (n == 0) return HCGRID_OK;
     ang2pix_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>((int)nside, n, lon, lat, pix);
@@ -69,7 +69,7 @@ int hcgrid_debug_ang2pix_ring(int64_t nside, int64_t n, const double* lon, const
 }
 
 int hcgrid_host_ang2pix_ring(int64_t nside, int64_t n, const double* lon, const double* lat, int64_t* pix) {
-    if (nside < 1 || nside > 8192 || (nside & (nside - 1)) || n < 0 || (n > 0 && (!lon || !lat || !pix)))
+    if (nside < 1 || nside > 16384 || (nside & (nside - 1)) || n < 0 || (n > 0 && (!lon || !lat || !pix)))
         return fail(nullptr, HCGRID_ERR_INVALID_ARG, "hcgrid_host_ang2pix_ring: bad arguments");
     for (int64_t i = 0; i < n; ++i) pix[i] = ang2pix_ring_deg((int)nside, lon[i], lat[i]);
     return HCGRID_OK;
@@ -77,7 +77,7 @@ int hcgrid_host_ang2pix_ring(int64_t nside, int64_t n, const double* lon, const 
 
 int hcgrid_host_ring_info(int64_t nside, int32_t iring, int64_t* first_pixel, int32_t* npix, double* lat_deg,
                           double* lon0_deg) {
-    if (nside < 1 || nside > 8192 || (nside & (nside - 1)) || iring < 1 || iring > 4 * nside - 1)
+    if (nside < 1 || nside > 16384 || (nside & (nside - 1)) || iring < 1 || iring > 4 * nside - 1)
         return fail(nullptr, HCGRID_ERR_INVALID_ARG, "hcgrid_host_ring_info: bad arguments");
     const int ns = (int)nside;
     if (first_pixel) *first_pixel = ring_first_pixel(iring, nside);

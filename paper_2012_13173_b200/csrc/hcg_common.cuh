@@ -157,6 +157,11 @@ struct hcgrid_ctx {
     hcg::DevBuf d_strips, d_wins, d_winsf, d_rowsf, d_cell_lon, d_cell_lat;
     double car_u0 = 0.0, car_du = 0.0;   // plate-carree target: lon offset of column 0 / column step, rad
     double car_dlat = 0.0;               // row step, rad (signed)
+    // the plate-carree target as the caller gave it, and the lookup-bin refinement chosen from the sample density
+    // (refine_target_for_density: auto sub-pixel bits only, -1000 = not refined)
+    int car_nx = 0, car_ny = 0;
+    double car_lon0_deg = 0.0, car_lat0_deg = 0.0, car_dlon_deg = 0.0, car_dlat_deg = 0.0;
+    int subpix_refined = -1000;
     double dlmax = 0.0;                  // widest longitude half-window of a support disc, rad
     bool tile_ok = false;                // the tile kernel's preconditions hold for this target
     // per-call scratch
@@ -204,6 +209,11 @@ namespace hcg {
 // stage entry points (defined in target.cu / preorder.cu / convolve*.cu)
 int build_target_car(hcgrid_ctx* c, int nx, int ny, double lon0, double lat0, double dlon, double dlat);
 int build_target_cells(hcgrid_ctx* c, int64_t ncell, const double* lon, const double* lat, cudaStream_t st);
+// Plate-carree targets with automatic sub-pixel bits: when the call brings more than 10 samples per lookup bin (the
+// radix-sort regime) and finer bins (towards 4 per bin, up to 2^6 per pixel) bring that to 10 or less, the tables are rebuilt --
+// the counting pre-order then applies and the search windows tighten.  Synchronises `st` and the device when it
+// rebuilds (once per target and density class); returns HCGRID_OK and *rebuilt.
+int refine_target_for_density(hcgrid_ctx* c, int64_t n, cudaStream_t st, bool* rebuilt);
 int run_preorder(hcgrid_ctx* c, int64_t n, const double* lon, const double* lat, const float* values,
                  int nchan, const float* weights, cudaStream_t st);
 int run_convolve(hcgrid_ctx* c, int64_t n, const float* values, int nchan, bool has_weights,

@@ -116,7 +116,7 @@ static int finish_target(hcgrid_ctx* c, const std::vector<HostStrip>& hs, int st
         npr_min = std::min(npr_min, ring_npix(r, nside));
     }
     // sub-pixel bits: auto = 2 (quarter-pixel bins), reduced until the table fits
-    int b = c->opt_subpix > -100 ? c->opt_subpix : 2;
+    int b = c->opt_subpix > -100 ? c->opt_subpix : (c->subpix_refined > -100 ? c->subpix_refined : 2);
     b = std::min(b, 6);
     const int64_t cap = (int64_t)1 << 28;
     for (;; --b) {
@@ -250,6 +250,8 @@ int build_target_car(hcgrid_ctx* c, int nx, int ny, double lon0, double lat0, do
     c->is_car = true;
     c->ncell = (int64_t)nx * ny;
     c->car_dlat = dlat * kDeg2Rad;
+    c->car_nx = nx; c->car_ny = ny;
+    c->car_lon0_deg = lon0; c->car_lat0_deg = lat0; c->car_dlon_deg = dlon; c->car_dlat_deg = dlat;
     return finish_target(c, hs, nx, std::min(a, b), std::max(a, b));
 }
 
@@ -303,6 +305,27 @@ static bool detect_car(const std::vector<double>& hl, const std::vector<double>&
     }
     nx = (int)w; ny = (int)h;
     return true;
+}
+
+int refine_target_for_density(hcgrid_ctx* c, int64_t n, cudaStream_t st, bool* rebuilt) {
+    *rebuilt = false;
+    const Region& rg = c->region;
+    if (!c->is_car || c->opt_subpix > -100 || rg.subpix >= 6 || n <= 10 * rg.nbins) return HCGRID_OK;
+    // finer bins double the table per bit: as many bits as bring the density down to 4 samples per bin -- or as many
+    // as there are -- while the per-ring table stays narrow enough for the tile kernels' fp32 bin arithmetic and the
+    // whole table modest; pointless if even that leaves more than 10 per bin (the radix path does not care about bins)
+    int b = rg.subpix;
+    int64_t nbins = rg.nbins, m = rg.m;
+    while (b < 6 && n > 4 * nbins && 2 * m < ((int64_t)1 << 22) && 2 * nbins <= ((int64_t)1 << 25)) { ++b; nbins *= 2; m *= 2; }
+    if (b == rg.subpix || n > 10 * nbins) return HCGRID_OK;
+    HCG_CUDA(c, cudaStreamSynchronize(st));                            // earlier calls may still read the tables
+    const int keep = c->subpix_refined;
+    c->subpix_refined = b;
+    const int rc = build_target_car(c, c->car_nx, c->car_ny, c->car_lon0_deg, c->car_lat0_deg, c->car_dlon_deg,
+                                    c->car_dlat_deg);
+    if (rc != HCGRID_OK) { c->subpix_refined = keep; return rc; }
+    *rebuilt = true;
+    return HCGRID_OK;
 }
 
 int build_target_cells(hcgrid_ctx* c, int64_t ncell, const double* lon, const double* lat, cudaStream_t st) {

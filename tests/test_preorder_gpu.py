@@ -160,3 +160,48 @@ def test_preorder_auto_choice():
     val = np.tile(w.values, (40, 1))
     st2 = _run_preorder_mode(w, binding.PREORDER_AUTO, lon=lon, lat=lat, values=val)[4]
     assert st2["preorder"] == (2 if lon.size <= 10 * st2["n_bins"] else 1)
+
+
+def test_dense_input_refines_the_lookup_bins(oracle):
+    """More than 10 samples per lookup bin on a plate-carree target with automatic sub-pixel bits: the first call
+    rebuilds the tables with finer bins, the counting pre-order applies, results match the oracle; a later sparse call
+    keeps the finer tables; an explicit HCGRID_OPT_SUBPIX_BITS or a new target switches it off / starts over."""
+    from paper_2012_13173_b200 import binding
+    from parity import TOL_F32, compare
+    rng = np.random.default_rng([13173, 4242])
+    n = 1_500_000
+    sigma, radius, nside = 127.4 / 3600.0, 382.2 / 3600.0, 2048
+    tgt = workloads.CarTarget(90, 90, 27.5, 22.5, 200.0 / 3600.0, 200.0 / 3600.0)
+    lon = 30.0 + rng.uniform(-2.5, 2.5, n)
+    lat = 25.0 + rng.uniform(-2.5, 2.5, n)
+    val = rng.standard_normal((n, 1)).astype(np.float32)
+    cl, cb = tgt.cell_centers()
+    cells = np.arange(0, tgt.ncell, 23)
+    ref = oracle.grid(sigma, radius, cl[cells], cb[cells], lon, lat, val, None)
+    d_lon, d_lat, d_val = _dev(lon), _dev(lat), _dev(val)
+    g = binding.HCGrid(sigma, radius, nside)
+    g.set_target_car(tgt.nx, tgt.ny, tgt.lon0, tgt.lat0, tgt.dlon, tgt.dlat)
+    g.grid(d_lon[:1000], d_lat[:1000], d_val[:1000])
+    s0 = g.stats()
+    assert s0["subpix_bits"] == 2 and n > 10 * s0["n_bins"]
+    for _ in range(2):                                   # the refining call and a plain one after it
+        cube, wmap, cnt = g.grid(d_lon, d_lat, d_val)
+        torch.cuda.synchronize()
+        s1 = g.stats()
+        assert s1["subpix_bits"] > 2 and s1["preorder"] == 2 and n <= 4 * s1["n_bins"] and s1["kernel"] == 6
+        compare(cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy(), ref, sigma, radius, TOL_F32, cells=cells)
+    g.grid(d_lon[:1000], d_lat[:1000], d_val[:1000])     # sparse again: the tables stay
+    assert g.stats()["subpix_bits"] == s1["subpix_bits"]
+    g.set_target_car(tgt.nx, tgt.ny, tgt.lon0, tgt.lat0, tgt.dlon, tgt.dlat)
+    g.grid(d_lon[:1000], d_lat[:1000], d_val[:1000])
+    assert g.stats()["subpix_bits"] == 2                 # a new target starts over
+    g.close()
+    g = binding.HCGrid(sigma, radius, nside)
+    g.set_option(binding.OPT_SUBPIX_BITS, 2)              # the caller's choice stands
+    g.set_target_car(tgt.nx, tgt.ny, tgt.lon0, tgt.lat0, tgt.dlon, tgt.dlat)
+    cube, wmap, cnt = g.grid(d_lon, d_lat, d_val)
+    torch.cuda.synchronize()
+    s2 = g.stats()
+    assert s2["subpix_bits"] == 2 and s2["preorder"] == 1
+    compare(cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy(), ref, sigma, radius, TOL_F32, cells=cells)
+    g.close()
