@@ -58,6 +58,8 @@ def main():
     gen = torch.Generator(device=dev)
     rows = []
     for n in sizes(args.nmax):
+        # a fresh target per size: the lookup-bin refinement a dense size triggers is not inherited by the next
+        g.set_target_car(NCELL_SIDE, NCELL_SIDE, LON_C - half, LAT_C - half, CELL_DEG, CELL_DEG)
         gen.manual_seed(13173 + n % 1000003)
         # positions uniform over the field (in coordinate degrees), generated on the device
         lon = LON_C + (torch.rand(n, dtype=torch.float64, device=dev, generator=gen) - 0.5) * FIELD_DEG
@@ -73,7 +75,29 @@ def main():
                 for k in keys:
                     acc[k].append(s[k])
         med = {k: float(np.median(v)) for k, v in acc.items()}
-        row = {"n": n, "us_total": med["us_total"], "us_convolve": med["us_convolve"],
+        # the call as a caller sees it (no per-stage events): back-to-back calls between two CUDA events, once with the
+        # graph replay of repeated calls (the default up to 2^21 samples) and once with eager launches
+        call = {}
+        reps = 50 if n <= 10 ** 6 else 5
+        for name, mode in (("us_call", -1), ("us_call_eager", 0)):
+            g.set_option(binding.OPT_PROFILE, 0)
+            g.set_option(binding.OPT_GRAPH, mode)
+            for _ in range(3):
+                g.grid(lon, lat, val, None, want_counts=False, out=out)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(reps):
+                g.grid(lon, lat, val, None, want_counts=False, out=out)
+            e1.record()
+            torch.cuda.synchronize()
+            call[name] = 1e3 * e0.elapsed_time(e1) / reps
+            call[name + "_graph"] = g.stats()["graph"]
+        g.set_option(binding.OPT_GRAPH, -1)
+        g.set_option(binding.OPT_PROFILE, 1)
+        row = {"n": n, "us_call": call["us_call"], "graph": call["us_call_graph"], "us_call_eager": call["us_call_eager"],
+               "subpix_bits": s["subpix_bits"], "preorder": s["preorder"],
+               "us_total": med["us_total"], "us_convolve": med["us_convolve"],
                "us_preorder": med["us_pixelise"] + med["us_sort"] + med["us_tables"] + med["us_pack"],
                "conv_share": med["us_convolve"] / med["us_total"], "samples_per_s": n / (med["us_total"] * 1e-6),
                "tile": f"{s['coarsen']}x{s['coarsen_y']}"}
