@@ -65,6 +65,11 @@ int hcgrid_create(hcgrid_ctx** out, double sigma_deg, double support_radius_deg,
         e = cudaEventCreate(&ev);
         if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaEventCreate"); }
     }
+    e = cudaEventCreateWithFlags(&c->ev_long, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaHostAlloc((void**)&c->h_long, 2 * sizeof(int32_t), cudaHostAllocMapped);
+    if (e == cudaSuccess) e = cudaHostGetDevicePointer((void**)&c->h_long_dev, c->h_long, 0);
+    if (e != cudaSuccess) { hcgrid_destroy(c); return cuda_fail(nullptr, e, "pinned word for the pre-order guard"); }
+    c->h_long[0] = c->h_long[1] = 0;
     KernelParams& kp = c->kp;
     kp.sigma = sigma_deg * kDeg2Rad;
     kp.radius = support_radius_deg * kDeg2Rad;
@@ -95,6 +100,8 @@ int hcgrid_destroy(hcgrid_ctx* c) {
     if (c->st_copy) cudaStreamDestroy(c->st_copy);
     if (c->st_comp) cudaStreamDestroy(c->st_comp);
     if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    if (c->ev_long) { cudaEventSynchronize(c->ev_long); cudaEventDestroy(c->ev_long); }
+    if (c->h_long) cudaFreeHost(c->h_long);
     if (c->st_cap) cudaStreamDestroy(c->st_cap);
     delete c;
     return HCGRID_OK;
@@ -201,6 +208,7 @@ int hcgrid_set_target_car(hcgrid_ctx* c, int32_t nx, int32_t ny, double lon0, do
     c->acc_nchan = 0;
     ++c->config_gen;
     c->subpix_refined = -1000;
+    c->force_radix = false;
     return build_target_car(c, nx, ny, lon0, lat0, dlon, dlat);
 }
 
@@ -214,6 +222,7 @@ int hcgrid_set_target_cells(hcgrid_ctx* c, int64_t ncell, const double* lon, con
     c->acc_nchan = 0;
     ++c->config_gen;
     c->subpix_refined = -1000;
+    c->force_radix = false;
     return build_target_cells(c, ncell, lon, lat, (cudaStream_t)stream);
 }
 

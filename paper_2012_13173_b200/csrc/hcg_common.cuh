@@ -162,6 +162,14 @@ struct hcgrid_ctx {
     int car_nx = 0, car_ny = 0;
     double car_lon0_deg = 0.0, car_lat0_deg = 0.0, car_dlon_deg = 0.0, car_dlat_deg = 0.0;
     int subpix_refined = -1000;
+    // Guard of the counting pre-order against piled-up input: bins beyond kLongBin samples are ordered one block per
+    // bin, which is slow when a large share of the samples sits in a few bins (a staring pointing).  Large calls copy
+    // the number of such bins and the longest one to the host behind themselves; once a call has seen more than 64 of
+    // them or one beyond 16 kLongBin samples, the following calls on this target take the radix sort (same S').
+    int32_t* h_long = nullptr;           // pinned, mapped [2]: written by order_long_kernel's last block
+    int32_t* h_long_dev = nullptr;       // its device address
+    cudaEvent_t ev_long = nullptr;
+    bool long_pending = false, force_radix = false;
     double dlmax = 0.0;                  // widest longitude half-window of a support disc, rad
     bool tile_ok = false;                // the tile kernel's preconditions hold for this target
     // per-call scratch

@@ -122,6 +122,7 @@ tables_pack_kernel(const uint32_t* __restrict__ skeys, const uint32_t* __restric
 // record on the way (a5).
 
 constexpr int kLongBin = 1024;           // bins longer than this are ordered by the block-sort kernel
+constexpr int64_t kGuardMinN = 1 << 20;  // calls from this size on report their count of such bins to the host
 constexpr uint32_t kStartFlag = 0x80000000u, kIdxMask = 0x7fffffffu;   // n <= 2e9 < 2^31 (hcgrid_grid)
 
 // sidx_raw[bin_start[key] + rank] = i, with the top bit set on rank 0: the sample that arrived
@@ -211,12 +212,13 @@ order_pack_kernel(const uint32_t* __restrict__ sidx_raw, int64_t n, const int32_
 template <bool kPack>
 __global__ void __launch_bounds__(256)
 order_long_kernel(const uint32_t* __restrict__ sidx_raw, const int32_t* __restrict__ bin_start,
-                  const int32_t* __restrict__ long_count, const int32_t* __restrict__ long_list, uint32_t* sidx,
-                  const Rec32* __restrict__ rec_in, Rec32* __restrict__ rec_out) {
+                  int32_t* __restrict__ long_count, const int32_t* __restrict__ long_list, uint32_t* sidx,
+                  const Rec32* __restrict__ rec_in, Rec32* __restrict__ rec_out, volatile int32_t* __restrict__ host_report) {
     const int nlong = long_count[0];
     for (int g = blockIdx.x; g < nlong; g += gridDim.x) {
         const int key = long_list[g];
         const int s = bin_start[key], len = bin_start[key + 1] - s;
+        if (threadIdx.x == 0) atomicMax(long_count + 1, len);   // the longest bin, for the host's guard (run_preorder)
         for (int k = threadIdx.x; k < len; k += 256) sidx[s + k] = sidx_raw[s + k] & kIdxMask;
         __syncthreads();
         block_sort_u32(sidx + s, len, threadIdx.x, 256);    // ends with a barrier
@@ -224,6 +226,15 @@ order_long_kernel(const uint32_t* __restrict__ sidx_raw, const int32_t* __restri
             for (int k = threadIdx.x; k < len; k += 256)
                 *(uint4*)(rec_out + s + k) = __ldg((const uint4*)(rec_in + sidx[s + k]));
         __syncthreads();
+    }
+    // the last block to leave tells the host (a mapped pinned word pair: no copy on the stream) how many bins came
+    // here and how long the longest was: run_preorder's guard against piled-up input reads it at a later call
+    if (host_report && threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(long_count + 2, 1) == (int)gridDim.x - 1) {
+            host_report[0] = nlong;
+            host_report[1] = ((volatile int32_t*)long_count)[1];
+        }
     }
 }
 
@@ -251,14 +262,27 @@ int run_preorder(hcgrid_ctx* c, int64_t n, const double* lon, const double* lat,
     // larger than the input (its O(bins) passes), or the option says otherwise; the result is
     // the same S' either way
     const int64_t nbins64 = (int64_t)rg.nbins;
+    // what an earlier large call on this target reported behind itself: bins too long for the counting path
+    // (event queries are not allowed while the thread captures a stream: the replay path asks later)
+    cudaStreamCaptureStatus capturing = cudaStreamCaptureStatusNone;
+    HCG_CUDA(c, cudaStreamIsCapturing(st, &capturing));
+    if (capturing != cudaStreamCaptureStatusNone || !c->long_pending) {
+        // nothing to read now
+    } else if (cudaEventQuery(c->ev_long) != cudaSuccess) {
+        cudaGetLastError();                                          // not ready: not an error
+    } else {
+        c->long_pending = false;
+        // a few bins of a few thousand samples are fine where they are; many, or a very long one, are not
+        if (c->h_long[0] > 64 || c->h_long[1] > 16 * kLongBin) c->force_radix = true;
+    }
     const bool counting = n > 0 && (c->opt_preorder == 2 ||
-                                    (c->opt_preorder == 0 && n <= 10 * nbins64 &&
+                                    (c->opt_preorder == 0 && !c->force_radix && n <= 10 * nbins64 &&
                                      (nbins64 <= 16 * n || nbins64 <= ((int64_t)1 << 22))));
     const size_t nn = (size_t)(n > 0 ? n : 1);
     HCG_CUDA(c, c->d_keys.ensure(nn * 4));
     HCG_CUDA(c, c->d_idx.ensure(nn * 4));
     HCG_CUDA(c, c->d_idx_out.ensure(nn * 4));
-    HCG_CUDA(c, c->d_bins.ensure(((size_t)rg.nbins + 2) * 4));
+    HCG_CUDA(c, c->d_bins.ensure(((size_t)rg.nbins + 4) * 4));   // + count of long bins, their largest length
     HCG_CUDA(c, c->d_rec.ensure(nn * (f32 ? sizeof(Rec32) : sizeof(Rec64)) + 64));
     if (f32) HCG_CUDA(c, c->d_misc.ensure(nn * sizeof(Rec32)));
     int end_bit = 1;
@@ -287,7 +311,7 @@ int run_preorder(hcgrid_ctx* c, int64_t n, const double* lon, const double* lat,
         uint32_t* rank = c->d_idx.as<uint32_t>();
         uint32_t* sidx_raw = c->d_keys_out.as<uint32_t>();   // arrival order, start-of-bin flags
         uint32_t* sidx = c->d_idx_out.as<uint32_t>();        // ascending inside every bin: the sorted "value" column
-        HCG_CUDA(c, cudaMemsetAsync(bins, 0, ((size_t)rg.nbins + 2) * 4, st));
+        HCG_CUDA(c, cudaMemsetAsync(bins, 0, ((size_t)rg.nbins + 4) * 4, st));
         if (f32)
             pixelise_kernel<true, true><<<nb, threads, 0, st>>>(lon, lat, values, weights, nchan, n, rg, keys, rank,
                                                                 c->d_misc.as<Rec32>(), bins);
@@ -304,18 +328,28 @@ int run_preorder(hcgrid_ctx* c, int64_t n, const double* lon, const double* lat,
         HCG_CUDA(c, cudaGetLastError());
         if (c->opt_profile) { cudaEventRecord(c->ev[2], st); cudaEventRecord(c->ev[3], st); }
         const unsigned nlb = (unsigned)(4 * c->num_sms);
+        // large calls report their long bins to the host behind themselves (never inside a stream capture: the event is
+        // queried by a later call)
+        volatile int32_t* report = nullptr;
+        if (n >= kGuardMinN && c->opt_preorder == 0 && !c->long_pending && c->h_long_dev &&
+            capturing == cudaStreamCaptureStatusNone)
+            report = c->h_long_dev;
         if (f32) {
             order_pack_kernel<true><<<nb, threads, 0, st>>>(sidx_raw, n, bins + rg.nbins, sidx, c->d_misc.as<Rec32>(),
                                                             c->d_rec.as<Rec32>());
             order_long_kernel<true><<<nlb, threads, 0, st>>>(sidx_raw, bins, long_count, long_list, sidx,
-                                                             c->d_misc.as<Rec32>(), c->d_rec.as<Rec32>());
+                                                             c->d_misc.as<Rec32>(), c->d_rec.as<Rec32>(), report);
         } else {
             order_pack_kernel<false><<<nb, threads, 0, st>>>(sidx_raw, n, bins + rg.nbins, sidx, nullptr, nullptr);
             order_long_kernel<false><<<nlb, threads, 0, st>>>(sidx_raw, bins, long_count, long_list, sidx, nullptr,
-                                                              nullptr);
+                                                              nullptr, report);
         }
         HCG_CUDA(c, cudaGetLastError());
         launches = 6;                        // pixelise, scan (2 kernels), scatter, order + pack, long bins
+        if (report) {
+            HCG_CUDA(c, cudaEventRecord(c->ev_long, st));
+            c->long_pending = true;
+        }
     } else {
         if (n > 0) {
             if (f32)

@@ -205,3 +205,53 @@ def test_dense_input_refines_the_lookup_bins(oracle):
     assert s2["subpix_bits"] == 2 and s2["preorder"] == 1
     compare(cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy(), ref, sigma, radius, TOL_F32, cells=cells)
     g.close()
+
+
+def test_piled_up_input_switches_later_calls_to_the_radix_sort(oracle):
+    """A tenth of 1.2 M samples within 1e-7 deg of one spot: the counting pre-order orders that bin one block at a
+    time (slow but right); the call reports it to the host behind itself and the following calls on the target take the
+    radix sort -- same S', same bits.  A few bins of a few thousand samples do not trigger it, a new target resets it."""
+    from paper_2012_13173_b200 import binding
+    from parity import TOL_F32, compare
+    w = workloads.make(3, 0.12)
+    t = w.target
+    rng = np.random.default_rng(99)
+    lon, lat = w.lon.copy(), w.lat.copy()
+    sel = rng.choice(w.n, w.n // 10, replace=False)
+    lon[sel] = t.lon0 + 0.37 * t.nx * t.dlon + rng.normal(0, 1e-7, sel.size)
+    lat[sel] = t.lat0 + 0.61 * t.ny * t.dlat + rng.normal(0, 1e-7, sel.size)
+    assert w.n >= 1 << 20
+    d = (_dev(lon), _dev(lat), _dev(w.values))
+    g = binding.HCGrid(w.sigma_deg, w.radius_deg, w.nside)
+    g.set_target_car(t.nx, t.ny, t.lon0, t.lat0, t.dlon, t.dlat)
+    res, pre = [], []
+    for _ in range(3):
+        r = g.grid(*d)
+        torch.cuda.synchronize()
+        res.append([x.clone() for x in r]); pre.append(g.stats()["preorder"])
+    assert pre == [2, 1, 1]
+    for a, b in zip(res[0], res[2]):
+        assert torch.equal(a.nan_to_num(nan=-1.0), b.nan_to_num(nan=-1.0))
+    cl, cb = t.cell_centers()
+    cells = np.arange(0, t.ncell, 97)
+    ref = oracle.grid(w.sigma_deg, w.radius_deg, cl[cells], cb[cells], lon, lat, w.values, None)
+    compare(res[2][0].cpu().numpy(), res[2][1].cpu().numpy(), res[2][2].cpu().numpy(), ref, w.sigma_deg, w.radius_deg,
+            TOL_F32, cells=cells)
+    g.set_target_car(t.nx, t.ny, t.lon0, t.lat0, t.dlon, t.dlat)          # a new target: the counting sort again
+    g.grid(*d)
+    assert g.stats()["preorder"] == 2
+    g.close()
+    # three bins of ~3000 samples: left to the block-sort kernel, no switch
+    lon2, lat2 = w.lon.copy(), w.lat.copy()
+    for k in range(3):
+        s2 = rng.choice(w.n, 3000, replace=False)
+        lon2[s2] = t.lon0 + (0.2 + 0.2 * k) * t.nx * t.dlon + rng.normal(0, 1e-7, s2.size)
+        lat2[s2] = t.lat0 + 0.5 * t.ny * t.dlat + rng.normal(0, 1e-7, s2.size)
+    d2 = (_dev(lon2), _dev(lat2), _dev(w.values))
+    g = binding.HCGrid(w.sigma_deg, w.radius_deg, w.nside)
+    g.set_target_car(t.nx, t.ny, t.lon0, t.lat0, t.dlon, t.dlat)
+    for _ in range(3):
+        g.grid(*d2)
+        torch.cuda.synchronize()
+        assert g.stats()["preorder"] == 2
+    g.close()
