@@ -196,6 +196,18 @@ def test_dense_input_refines_the_lookup_bins(oracle):
     g.grid(d_lon[:1000], d_lat[:1000], d_val[:1000])
     assert g.stats()["subpix_bits"] == 2                 # a new target starts over
     g.close()
+    # two dense batches through hcgrid_accumulate on a fresh context: the first one refines, the sums do not care
+    g = binding.HCGrid(sigma, radius, nside)
+    g.set_target_car(tgt.nx, tgt.ny, tgt.lon0, tgt.lat0, tgt.dlon, tgt.dlat)
+    h = n - n // 8                                        # 1.3 M samples: still more than 10 per quarter-pixel bin
+    g.accumulate(d_lon[:h], d_lat[:h], d_val[:h])
+    b1 = g.stats()["subpix_bits"]
+    g.accumulate(d_lon[h:], d_lat[h:], d_val[h:])
+    cube, wmap, cnt = g.finalize()
+    torch.cuda.synchronize()
+    assert b1 > 2 and g.stats()["subpix_bits"] == b1
+    compare(cube.cpu().numpy(), wmap.cpu().numpy(), cnt.cpu().numpy(), ref, sigma, radius, TOL_F32, cells=cells)
+    g.close()
     g = binding.HCGrid(sigma, radius, nside)
     g.set_option(binding.OPT_SUBPIX_BITS, 2)              # the caller's choice stands
     g.set_target_car(tgt.nx, tgt.ny, tgt.lon0, tgt.lat0, tgt.dlon, tgt.dlat)
