@@ -59,9 +59,11 @@ constexpr int kTcGroups = 16;                  // FIFO groups
 constexpr int kTcFifo = kTcGroups * kTcSC;     // FIFO entries
 constexpr int kTcRings = 128;                  // ring-table entries per pass
 constexpr int kBrawBytes = kTcKS * 8192;       // spectrum rows of a stage: kTcKS K-steps x 8 rows x 1 KB
-constexpr int kOffBraw = 0, kOffBlo = kBrawBytes, kStageBytes = 2 * kBrawBytes;
+// ... and their low parts v - trunc_tf32(v) in bf16, one 8 KB tile (16 rows x 256 channels) per pair of K-steps
+constexpr int kBloBytes = (kTcKS / 2) * 8192;
+constexpr int kOffBraw = 0, kOffBlo = kBrawBytes, kStageBytes = kBrawBytes + kBloBytes;
 constexpr int kTmemA = 256;                    // TMEM columns: accumulator 0 .. 255, A ring from 256
-constexpr int kTmemAStage = 16 * kTcKS;        // per stage: hi kTcKS x 8 columns, then lo kTcKS x 8 columns
+constexpr int kTmemAStage = 16 * kTcKS + 8 * (kTcKS / 2);   // per stage: hi kTcKS x 8 columns, lo kTcKS x 8, then the weights in bf16: kTcKS / 2 x 8
 static_assert(kTmemA + kTcNS * kTmemAStage <= 512, "TMEM columns");
 // FIFO: per pair of candidates three float4: (Xh_a, Xh_b, Xl_a, Xl_b), (Yh_a, Yh_b, Yl_a, Yl_b), (cs_a, cs_b, q_a, q_b)
 constexpr int kOffFifoX = kTcNS * kStageBytes;
@@ -205,6 +207,25 @@ __device__ __forceinline__ uint32_t umma_idesc_tf32(int n) {
     return (1u << 4) | (2u << 7) | (2u << 10) | (0u << 15) | (1u << 16) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
 }
 
+// the same for kind::f16 on bf16 operands (A K-major from tensor memory, B MN-major)
+__device__ __forceinline__ uint32_t umma_idesc_bf16(int n) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | (0u << 15) | (1u << 16) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+}
+__device__ __forceinline__ void umma_bf16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+                 ::"r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
+}
+// two floats rounded to bf16 and packed: `lo` in the low half
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+    uint32_t d;
+    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
+    return d;
+}
+__device__ __forceinline__ void sts_u2(uint32_t addr, uint32_t a, uint32_t b) {
+    asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(addr), "r"(a), "r"(b) : "memory");
+}
+
 template <int MODE, bool COUNTS>
 __global__ void __launch_bounds__(kTcThreads, 1)
 conv_mc_tc_f32(const McTcArgs m) {
@@ -261,7 +282,10 @@ conv_mc_tc_f32(const McTcArgs m) {
         if (warp == kMmaWarp) {
             // ============================================================ MMA issuer (lane 0 issues; the warp stays converged)
             const uint32_t idesc = umma_idesc_tf32(nch);
-            const uint64_t b_rw0 = umma_desc(s_base + kOffBraw, 1024, 512, 1), b_lo0 = umma_desc(s_base + kOffBlo, 1024, 512, 1);
+            const uint32_t idesc16 = umma_idesc_bf16(nch);
+            // spectrum rows: 32-bit MN-major, SWIZZLE_128B_BASE32B; their low parts: bf16 MN-major, SWIZZLE_128B (64-channel
+            // segments 2048 bytes apart, the two 8-row groups of a 16-row tile 1024 bytes apart)
+            const uint64_t b_rw0 = umma_desc(s_base + kOffBraw, 1024, 512, 1), b_lo0 = umma_desc(s_base + kOffBlo, 2048, 1024, 2);
             for (int s = 0;; ++s) {
                 const int slot = s % kTcNS;
                 const uint32_t par = (uint32_t)(s / kTcNS) & 1u;
@@ -276,12 +300,16 @@ conv_mc_tc_f32(const McTcArgs m) {
                     if (lane == 0) {
                         const uint64_t so = (uint64_t)((uint32_t)slot * (kStageBytes >> 4));
 #pragma unroll
-                        for (int ks = 0; ks < kTcKS; ++ks) {
+                        for (int ks = 0; ks < kTcKS; ++ks) {               // w_hi * v + w_lo * v, TF32 (the unit truncates v)
                             const uint32_t ah = tm + kTmemA + (uint32_t)(slot * kTmemAStage + ks * 8), al = ah + 8 * kTcKS;
-                            const uint64_t br = b_rw0 + so + (uint64_t)(ks * (8192 >> 4)), bl = b_lo0 + so + (uint64_t)(ks * (8192 >> 4));
+                            const uint64_t br = b_rw0 + so + (uint64_t)(ks * (8192 >> 4));
                             umma_tf32_ts(tm, ah, br, idesc, (first && ks == 0) ? 0u : 1u);
                             umma_tf32_ts(tm, al, br, idesc, 1u);
-                            umma_tf32_ts(tm, ah, bl, idesc, 1u);
+                        }
+#pragma unroll
+                        for (int j = 0; j < kTcKS / 2; ++j) {              // + w * v_lo: a 2^-11 term, bf16 x bf16 over 16 candidates
+                            const uint32_t ab = tm + kTmemA + (uint32_t)(slot * kTmemAStage + 16 * kTcKS + j * 8);
+                            umma_bf16_ts(tm, ab, b_lo0 + so + (uint64_t)(j * (8192 >> 4)), idesc16, 1u);
                         }
                         tc_commit(b_empty + 8 * slot);
                         if (s % kTcCH == kTcCH - 1 || (flag & 1u)) tc_commit(b_dfull);
@@ -501,6 +529,16 @@ conv_mc_tc_f32(const McTcArgs m) {
         const uint32_t fifo_i_s = s_base + kOffFifoI, grp_n_s = s_base + kOffGrpN;
         // row r = 2 i + rp of the stage: (r >> 3) = i >> 2, (r >> 2) & 1 = (i >> 1) & 1, r & 3 = 2 (i & 1) + rp
         auto unit_off = [&](int i) -> uint32_t { return (uint32_t)((i >> 2) * 8192 + ((i >> 1) & 1) * 512) + off_u[i & 1]; };
+        // the 8 bytes (4 channels in bf16) of the same unit in the low-part tiles: row r = 2 i + rp is row k = r & 15 of tile
+        // r >> 4; channels 4 u ..: segment u >> 4 (2048 bytes), 8-row group k >> 3 (1024), row k & 7 (128), 16-byte chunk
+        // ((u & 15) >> 1) ^ (k & 7), half u & 1
+        uint32_t off_l[4];                                            // by i & 3 (= the row's k & 7 given rp)
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+            const int k7 = 2 * v + rp;
+            off_l[v] = (uint32_t)((u >> 4) * 2048 + k7 * 128 + ((((u & 15) >> 1) ^ k7) << 4) + (u & 1) * 8);
+        }
+        auto lo_off = [&](int i) -> uint32_t { return (uint32_t)((i >> 3) * 8192 + ((i >> 2) & 1) * 1024) + off_l[i & 3]; };
         constexpr int NU = kTcSC / 2;                                 // units per thread per stage
         int nst = 0x7fffffff, pf = 0;
         for (int k = 0;; ++k) {
@@ -552,12 +590,11 @@ conv_mc_tc_f32(const McTcArgs m) {
                 auto split4 = [&](uint4 (&v)[4], int i0) {
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {
-                        uint4 l;
-                        l.x = __float_as_uint(__uint_as_float(v[j].x) - __uint_as_float(v[j].x & 0xffffe000u));
-                        l.y = __float_as_uint(__uint_as_float(v[j].y) - __uint_as_float(v[j].y & 0xffffe000u));
-                        l.z = __float_as_uint(__uint_as_float(v[j].z) - __uint_as_float(v[j].z & 0xffffe000u));
-                        l.w = __float_as_uint(__uint_as_float(v[j].w) - __uint_as_float(v[j].w & 0xffffe000u));
-                        sts_u4(sb + (kOffBlo - kOffBraw) + unit_off(i0 + j), l);
+                        const float lx = __uint_as_float(v[j].x) - __uint_as_float(v[j].x & 0xffffe000u);
+                        const float ly = __uint_as_float(v[j].y) - __uint_as_float(v[j].y & 0xffffe000u);
+                        const float lz = __uint_as_float(v[j].z) - __uint_as_float(v[j].z & 0xffffe000u);
+                        const float lw = __uint_as_float(v[j].w) - __uint_as_float(v[j].w & 0xffffe000u);
+                        sts_u2(sb + (kOffBlo - kOffBraw) + lo_off(i0 + j), pack_bf16(lx, ly), pack_bf16(lz, lw));
                     }
                 };
                 uint4 va[4], vb[4];
@@ -682,6 +719,14 @@ conv_mc_tc_f32(const McTcArgs m) {
                     lo[2 * pp + 1] = __float_as_uint(wb - __uint_as_float(hi[2 * pp + 1]));
                 }
                 const uint32_t t_hi = t_lane + kTmemA + (uint32_t)(slot * kTmemAStage + ks * 8), t_lo = t_hi + 8 * kTcKS;
+                // the same eight weights in bf16 for the low-part product: candidates 8 kk .. 8 kk + 7 of this thread's
+                // 16-candidate tile g = columns 4 kk .. 4 kk + 3 (column c: candidate 2 c in the low half, 2 c + 1 in the high)
+                const uint32_t t_bf = t_lane + kTmemA + (uint32_t)(slot * kTmemAStage + 16 * kTcKS + g * 8 + kk * 4);
+                asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};"
+                             ::"r"(t_bf), "r"(pack_bf16(__uint_as_float(hi[0]), __uint_as_float(hi[1]))),
+                               "r"(pack_bf16(__uint_as_float(hi[2]), __uint_as_float(hi[3]))),
+                               "r"(pack_bf16(__uint_as_float(hi[4]), __uint_as_float(hi[5]))),
+                               "r"(pack_bf16(__uint_as_float(hi[6]), __uint_as_float(hi[7]))) : "memory");
                 asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
                              ::"r"(t_hi), "r"(hi[0]), "r"(hi[1]), "r"(hi[2]), "r"(hi[3]), "r"(hi[4]), "r"(hi[5]), "r"(hi[6]), "r"(hi[7]) : "memory");
                 asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
