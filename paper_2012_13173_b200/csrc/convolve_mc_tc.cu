@@ -20,13 +20,16 @@
 //     shared-memory round trip and no proxy fence on this path;
 //   * 4 spectrum-row warps copy the candidates' spectrum rows IN PLACE from `values` (never moved: a5)
 //     with cp.async into the UMMA MN-major SWIZZLE_128B_BASE32B layout, a stage ahead, and write
-//     lo = v - trunc_tf32(v) beside them (the tensor core itself ignores the low 13 bits of v);
-//   * MMA warp: one thread issues, per 8 candidates, three tcgen05.mma.kind::tf32 (hi*v, lo*v, hi*lo_v:
-//     3xTF32, product error <= ~3e-6 relative) into a 128 x 256 fp32 accumulator in TMEM.
+//     v_lo = v - trunc_tf32(v) in bf16 into half-size MN-major SWIZZLE_128B tiles beside them (the tensor
+//     core itself ignores the low 13 bits of v);
+//   * MMA warp: one thread issues, per 8 candidates, two tcgen05.mma.kind::tf32 (w_hi * v, w_lo * v) and,
+//     per 16 candidates, one kind::f16 on bf16 operands (w * v_lo: a 2^-11 term, for which 2^-9 of itself
+//     is accuracy enough) into a 128 x 256 fp32 accumulator in TMEM: product error <= ~3e-6 relative.
 // The tensor core adds with round-toward-zero (measured: -3.4e-8 relative per update), so the TMEM
-// accumulator only ever holds a CHUNK of 4 stages (48 updates): the compute warps add every finished
-// chunk into fp32 registers (round-to-nearest, 128 channels x 1 cell per thread), which also makes the
-// epilogue a plain divide and store.  W and the counts are summed on the CUDA cores from the same
+// accumulator only ever holds a CHUNK of 8 stages (80 updates, bias <= 2.7e-6): the compute warps add every
+// finished chunk into fp32 registers (round-to-nearest, 128 channels x 1 cell per thread), which also makes
+// the epilogue a plain scale and store.  (4 stages per chunk: 1.6e-6 and 10 % slower; 10 and more: no faster.)
+// W and the counts are summed on the CUDA cores from the same
 // weights.  No atomics in the sums; the order of the additions is fixed by the stream order, so results
 // are bit-wise reproducible.
 // Odd tile rows walk the rings south to north, so vertically adjacent tiles, which run at the same
@@ -54,7 +57,7 @@ constexpr int kTcKS = 4;                       // K-steps (of 8 candidates) per 
 constexpr int kTcSC = 8 * kTcKS;               // candidates per stage = per FIFO group
 constexpr int kTcNS = 3;                       // pipeline stages (B in shared memory, A in tensor memory)
 constexpr int kTcBD = 1;                       // stages the spectrum rows are requested ahead of their split
-constexpr int kTcCH = 4;                       // stages per TMEM accumulator chunk (3 kTcKS kTcCH updates)
+constexpr int kTcCH = 8;                       // stages per TMEM accumulator chunk (10 MMA updates per stage)
 constexpr int kTcGroups = 16;                  // FIFO groups
 constexpr int kTcFifo = kTcGroups * kTcSC;     // FIFO entries
 constexpr int kTcRings = 128;                  // ring-table entries per pass
