@@ -43,7 +43,7 @@ UNIT = "cell-channels/s"
 NCU_TRAFFIC = {
     (3, 6): (191993856 + 12059648, "profiles/r02_conv1_tile_ncu_full.md"),
     (4, 7): (3714980000 + 98979072, "profiles/r01c_conv_mc_ncu_full.md"),
-    (4, 8): (1365308000 + 83858944, "profiles/r02_conv_mc_tc_ncu_full.md"),
+    (4, 8): (1360306000 + 82240256, "profiles/r02_conv_mc_tc_ncu_full.md"),
 }
 WORKLOAD_NAMES = {1: "config1_tiny_20k", 2: "config2_drift_scan_1.25M", 3: "config3_dense_10M",
                   4: "config4_spectral_cube_1M_x256", 5: "config5_polar_20M"}
