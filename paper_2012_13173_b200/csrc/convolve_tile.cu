@@ -27,8 +27,10 @@ namespace hcg {
 constexpr int kTileWarps = 4;        // warps (= tiles) per CTA when tiles are not split
 constexpr int kMaxTileWarps = 4;     // largest split: warps of one CTA on one tile
 
+// 8-cell Gaussian tiles without the count output fit 64 registers in every series mode (8 CTAs per SM) once ptxas is
+// asked to; left to itself it takes 71-72 for the series modes (0 = no request for the other variants).
 template <int GX, int GY, int MODE, bool COUNTS, bool SPLIT, int KFN = 0>
-__global__ void __launch_bounds__(kMaxTileWarps * 32)
+__global__ void __launch_bounds__(kMaxTileWarps * 32, (!COUNTS && KFN == 0 && GX * GY == 8) ? 8 : 0)
 conv1_tile_f32(const TileArgs a) {
     constexpr int NC = GX * GY;
     __shared__ unsigned long long s_tab[kMaxTileWarps][32];
