@@ -101,6 +101,16 @@ def test_anything_a_launch_depends_on_ends_the_replay(oracle):
     out_nc = (out[0], out[1], None)                                     # without the count output
     r, gr = call(out=out_nc, want_counts=False); assert gr == 0; check(r)
     r, gr = call(out=out_nc, want_counts=False); assert gr == 1; check(r)
+    g.set_kernel(binding.KERNEL_ELLIPTICAL_GAUSS, 0.5, 30.0)            # another kernel function
+    r, gr = call(out=out_nc, want_counts=False); assert gr == 0
+    cl, cb = t.cell_centers()
+    ref_e = oracle.grid(w.sigma_deg, w.radius_deg, cl, cb, w.lon, w.lat, w.values, None,
+                        kernel=(oracle.ELLIPTICAL_GAUSS, 0.5, 30.0))
+    compare(r[0].cpu().numpy(), r[1].cpu().numpy(), None, ref_e, w.sigma_deg, w.radius_deg, TOL_F32)
+    r, gr = call(out=out_nc, want_counts=False); assert gr == 1
+    compare(r[0].cpu().numpy(), r[1].cpu().numpy(), None, ref_e, w.sigma_deg, w.radius_deg, TOL_F32)
+    g.set_kernel(binding.KERNEL_GAUSS)
+    r, gr = call(out=out_nc, want_counts=False); assert gr == 0; check(r)
     g.set_target_car(t.nx, t.ny, t.lon0, t.lat0, t.dlon, t.dlat)       # a new target, even if equal
     r, gr = call(out=out_nc, want_counts=False); assert gr == 0; check(r)
     g.set_option(binding.OPT_PROFILE, 1)                               # per-stage events need an eager call
